@@ -1,0 +1,173 @@
+"""CPU oracle of the geometry-guidance hot path — TEST INFRASTRUCTURE, not the product.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs import this.
+The arithmetic lives in ggt_oracle.cpp (plain single-threaded C++, written from PAPER.md); this file
+only compiles it with g++ and marshals numpy arrays.  It imports nothing from the CUDA package
+except never: the two sides share no code.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "ggt_oracle.cpp")
+_LIB = os.path.join(_HERE, "libggt_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle (g++ -O2, contraction off, no fast-math)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp%d" % os.getpid()
+        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
+                               "-o", tmp, _SRC])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class OrcCamera(ctypes.Structure):
+    _fields_ = [("fx", ctypes.c_float), ("fy", ctypes.c_float), ("cx", ctypes.c_float),
+                ("cy", ctypes.c_float), ("R", ctypes.c_float * 9), ("t", ctypes.c_float * 3),
+                ("width", ctypes.c_int32), ("height", ctypes.c_int32)]
+
+
+def _cam(c) -> OrcCamera:
+    o = OrcCamera()
+    o.fx, o.fy, o.cx, o.cy = c.fx, c.fy, c.cx, c.cy
+    o.R[:] = [float(x) for x in np.asarray(c.R, dtype=np.float32).reshape(9)]
+    o.t[:] = [float(x) for x in np.asarray(c.t, dtype=np.float32).reshape(3)]
+    o.width, o.height = int(c.width), int(c.height)
+    return o
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+        _lib.orc_round_f16.restype = ctypes.c_float
+        _lib.orc_round_f16.argtypes = [ctypes.c_float]
+    return _lib
+
+
+def _p(a, ty):
+    return a.ctypes.data_as(ctypes.POINTER(ty)) if a is not None else None
+
+
+def round_f16(x: float) -> float:
+    return float(_load().orc_round_f16(ctypes.c_float(x)))
+
+
+def refine(rgb_cur, rgb_prev, depth_cur, depth_state, lambda_t=0.7, beta=0.6, theta=0.0,
+           downscale=4, pool=3, want_mask=True):
+    """O-R. Returns (refined depth, mask or None, pooled uint16 or None, binary uint8 or None)."""
+    lib = _load()
+    H, W = depth_cur.shape
+    depth_cur = np.ascontiguousarray(depth_cur, dtype=np.float32)
+    state = np.array(depth_state, dtype=np.float32, order="C", copy=True)
+    mask = np.empty((H, W), dtype=np.float32) if want_mask else None
+    pooled = binary = None
+    stride = 3
+    if rgb_prev is not None:
+        rgb_cur = np.ascontiguousarray(rgb_cur, dtype=np.uint8)
+        rgb_prev = np.ascontiguousarray(rgb_prev, dtype=np.uint8)
+        stride = rgb_cur.shape[2]
+        Hq, Wq = -(-H // downscale), -(-W // downscale)
+        pooled = np.empty((Hq, Wq), dtype=np.uint16)
+        binary = np.empty((Hq, Wq), dtype=np.uint8)
+    rc = lib.orc_refine(ctypes.c_int32(W), ctypes.c_int32(H), _p(rgb_cur, ctypes.c_uint8),
+                        _p(rgb_prev, ctypes.c_uint8), ctypes.c_int32(stride),
+                        _p(depth_cur, ctypes.c_float), _p(state, ctypes.c_float), _p(mask, ctypes.c_float),
+                        _p(pooled, ctypes.c_uint16), _p(binary, ctypes.c_uint8),
+                        ctypes.c_float(lambda_t), ctypes.c_float(beta), ctypes.c_float(theta),
+                        ctypes.c_int32(downscale), ctypes.c_int32(pool))
+    if rc != 0:
+        raise ValueError("orc_refine rc=%d" % rc)
+    return state, mask, pooled, binary
+
+
+def weight_map(depth, sigma0=0.001, clip=0.02, window=7) -> np.ndarray:
+    """O-W. Returns (H, W, 2) float32 interleaved {depth, omega}."""
+    lib = _load()
+    depth = np.ascontiguousarray(depth, dtype=np.float32)
+    H, W = depth.shape
+    out = np.empty((H, W, 2), dtype=np.float32)
+    rc = lib.orc_weight_map(ctypes.c_int32(W), ctypes.c_int32(H), _p(depth, ctypes.c_float),
+                            _p(out, ctypes.c_float), ctypes.c_float(sigma0), ctypes.c_float(clip),
+                            ctypes.c_int32(window))
+    if rc != 0:
+        raise ValueError("orc_weight_map rc=%d" % rc)
+    return out
+
+
+def tau_table(z_bins, trunc_bins=2.0, trunc_metric=0.0) -> np.ndarray:
+    lib = _load()
+    z = np.ascontiguousarray(z_bins, dtype=np.float32)
+    tau = np.empty_like(z)
+    rc = lib.orc_tau_table(ctypes.c_int32(z.size), _p(z, ctypes.c_float), ctypes.c_float(trunc_bins),
+                           ctypes.c_float(trunc_metric), _p(tau, ctypes.c_float))
+    if rc != 0:
+        raise ValueError("orc_tau_table rc=%d" % rc)
+    return tau
+
+
+def relative(target, view):
+    lib = _load()
+    Hm = np.empty(9, dtype=np.float32)
+    e = np.empty(3, dtype=np.float32)
+    t, v = _cam(target), _cam(view)
+    lib.orc_relative(ctypes.byref(t), ctypes.byref(v), _p(Hm, ctypes.c_float), _p(e, ctypes.c_float))
+    return Hm.reshape(3, 3), e
+
+
+def integrate(target, z_bins, tau, views: Sequence, maps: Sequence[np.ndarray],
+              rays: Optional[np.ndarray] = None, T: Optional[np.ndarray] = None,
+              Wt: Optional[np.ndarray] = None, accumulate=False, decay=1.0, cap=64.0,
+              half_storage=False):
+    """O-I. Returns (T, W) arrays of shape (n_rays, D); n_rays = H_t*W_t when rays is None."""
+    lib = _load()
+    z = np.ascontiguousarray(z_bins, dtype=np.float32)
+    tau = np.ascontiguousarray(tau, dtype=np.float32)
+    D = z.size
+    n_rays = int(target.width) * int(target.height) if rays is None else int(rays.size)
+    if rays is not None:
+        rays = np.ascontiguousarray(rays, dtype=np.int32)
+    if T is None:
+        T = np.zeros((n_rays, D), dtype=np.float32)
+        Wt = np.zeros((n_rays, D), dtype=np.float32)
+    else:
+        T = np.array(T, dtype=np.float32, order="C", copy=True).reshape(n_rays, D)
+        Wt = np.array(Wt, dtype=np.float32, order="C", copy=True).reshape(n_rays, D)
+    V = len(views)
+    cams = (OrcCamera * max(V, 1))(*[_cam(c) for c in views])
+    maps = [np.ascontiguousarray(m, dtype=np.float32) for m in maps]
+    ptrs = (ctypes.POINTER(ctypes.c_float) * max(V, 1))(*[_p(m, ctypes.c_float) for m in maps])
+    t = _cam(target)
+    rc = lib.orc_integrate(ctypes.byref(t), ctypes.c_int32(D), _p(z, ctypes.c_float), _p(tau, ctypes.c_float),
+                           ctypes.c_int32(V), cams, ptrs, ctypes.c_int64(n_rays), _p(rays, ctypes.c_int32),
+                           _p(T, ctypes.c_float), _p(Wt, ctypes.c_float), ctypes.c_int32(int(accumulate)),
+                           ctypes.c_float(decay), ctypes.c_float(cap), ctypes.c_int32(int(half_storage)))
+    if rc != 0:
+        raise ValueError("orc_integrate rc=%d" % rc)
+    return T, Wt
+
+
+def extract(z_bins, T, Wt):
+    """O-E. Returns (depth, conf, bin) per ray."""
+    lib = _load()
+    z = np.ascontiguousarray(z_bins, dtype=np.float32)
+    T = np.ascontiguousarray(T, dtype=np.float32)
+    Wt = np.ascontiguousarray(Wt, dtype=np.float32)
+    n_rays, D = T.shape
+    depth = np.empty(n_rays, dtype=np.float32)
+    conf = np.empty(n_rays, dtype=np.float32)
+    bins = np.empty(n_rays, dtype=np.int32)
+    lib.orc_extract(ctypes.c_int64(n_rays), ctypes.c_int32(D), _p(z, ctypes.c_float), _p(T, ctypes.c_float),
+                    _p(Wt, ctypes.c_float), _p(depth, ctypes.c_float), _p(conf, ctypes.c_float),
+                    _p(bins, ctypes.c_int32))
+    return depth, conf, bins
