@@ -1,0 +1,170 @@
+/* ggt.h — C ABI of the B200-native geometry-guidance hot path of arxiv/paper_2505_18932
+ * ("Geometry-guided Online 3D Video Synthesis with Multi-View Temporal Consistency").
+ *
+ * Three calls follow the paper's statement of the problem (PAPER.md:59 inputs, :96 output):
+ *   ggt_refine_depth   colour-difference-mask temporal refinement of ONE input depth map
+ *                      (Eq. 1-2)
+ *   ggt_integrate      target camera + V input cameras / depth maps -> TSDF + weight volume laid out in
+ *                      the target view's image space (pixel u,v x depth bin), overwrite or persistent
+ *                      (Eq. 9-12; persistence: analogue of Eq. 13-14)
+ *   ggt_extract_depth  volume -> per-pixel zero-crossing depth + confidence
+ *
+ * Conventions
+ *   - every call returns int: GGT_OK (0) or a negative GGT_ERR_*; ggt_last_error() gives the text.
+ *   - arguments named dev_* are DEVICE pointers owned by the caller (e.g. torch tensors); the library
+ *     never frees them.  Camera structs, descriptor structs and pointer arrays are HOST memory, copied
+ *     at call time.  Arguments named host_* are host pointers (pinned memory makes the copies async).
+ *   - `stream` is the caller's cudaStream_t passed as void* (NULL = legacy default stream).  Calls
+ *     validate host-side arguments synchronously, enqueue kernels on `stream` and return WITHOUT
+ *     synchronising.  No exception crosses the ABI.
+ *   - there is no CPU fallback: without a CUDA device every compute call returns GGT_ERR_CUDA.
+ *   - depth maps hold z-depth in metres (the quantity Eq. 9 compares with z_k); <= 0 means invalid.
+ *   - pixel (i, j) has its centre at (i + 0.5, j + 0.5); images are row-major, row 0 on top.
+ *   - arithmetic is IEEE fp32 in a fixed operation order (P14), so
+ *     results are bit-reproducible and comparable with the oracle on the discrete decisions.
+ */
+#ifndef GGT_H_
+#define GGT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GGT_OK 0
+#define GGT_ERR_INVALID_ARG (-1)
+#define GGT_ERR_SHAPE (-2)
+#define GGT_ERR_UNSUPPORTED (-3)
+#define GGT_ERR_CUDA (-4)
+
+#define GGT_F32 0          /* volume storage: {T, W} as 2 x fp32 = 8 B / voxel */
+#define GGT_F16 1          /* volume storage: {T, W} as 2 x fp16 = 4 B / voxel (RNE on store) */
+
+#define GGT_OVERWRITE 0u   /* T = sum(w c)/sum(w), W = sum(w)  (Eq. 10, normalised: reading P2) */
+#define GGT_ACCUMULATE 1u  /* running average against the stored {T, W} with decay and cap (P9) */
+
+#define GGT_MAX_VIEWS 16
+#define GGT_MAX_BINS 1024
+
+/* Pinhole camera, no skew / distortion.  x_cam = R p_world + t. */
+typedef struct ggt_camera {
+    float fx, fy, cx, cy;
+    float R[9];            /* row-major */
+    float t[3];
+    int32_t width, height;
+} ggt_camera;
+
+/* Eq. 1 parameters.  Paper: lambda_t = 0.7, beta = 0.6, theta = 0;
+ * BASELINE.json:configs[2] adds the dead zone theta = 8/255 (reading P6).
+ * Only downscale = 4 and pool = 3 (the paper's values) are implemented: others -> GGT_ERR_UNSUPPORTED. */
+typedef struct ggt_refine_params {
+    float lambda_t, beta, theta;
+    int32_t downscale, pool;
+} ggt_refine_params;
+
+/* Volume descriptor.  tau_j = trunc_bins x local bin spacing (reading P3) unless trunc_metric > 0
+ * (paper: 0.02 m).  w_window = 7, w_sigma0 = 0.001, w_clip = 0.02 are Eq. 11-12's
+ * constants; w_window = 0 gives omega = 1 on valid pixels.  weight_cap / decay: persistent mode. */
+typedef struct ggt_volume_desc {
+    int32_t width, height, bins;   /* W_t, H_t, D (2 <= D <= GGT_MAX_BINS) */
+    const float* z_bins;           /* HOST, D strictly increasing z-depths (metres) */
+    float trunc_bins;
+    float trunc_metric;
+    float w_sigma0, w_clip;
+    int32_t w_window;              /* 0 or 7 */
+    float weight_cap, decay;
+    int32_t dtype;                 /* GGT_F32 | GGT_F16 */
+} ggt_volume_desc;
+
+typedef struct ggt_ctx ggt_ctx;
+typedef struct ggt_volume ggt_volume;
+
+/* ---- context ------------------------------------------------------------------------------------ */
+/* Creates a context on the current CUDA device.  GGT_ERR_CUDA if there is none. */
+int ggt_create(ggt_ctx** out);
+int ggt_destroy(ggt_ctx* ctx);
+/* Text of the last error on this context (or of the last ggt_create failure if ctx == NULL). */
+const char* ggt_last_error(const ggt_ctx* ctx);
+/* Number of kernels this context has launched so far (bench.py's gpu_launches). */
+int64_t ggt_launch_count(const ggt_ctx* ctx);
+
+/* ---- workspace for the {depth, omega} maps of Eq. 11-12 ------------------------------------------ */
+/* Bytes of device scratch ggt_integrate needs for n_views maps of width x height: 8 B per pixel. */
+size_t ggt_workspace_bytes(int32_t n_views, int32_t width, int32_t height);
+/* Hands caller-owned device scratch to the context.  Without it (or if it is too small) ggt_integrate
+ * grows an internal cudaMalloc'ed buffer, which synchronises the device once per growth. */
+int ggt_set_workspace(ggt_ctx* ctx, void* dev_workspace, size_t bytes);
+
+/* ---- volume ------------------------------------------------------------------------------------- */
+/* Bytes the caller must allocate for a volume: a 256-B-aligned table header (z_j, tau_j) followed by
+ * the voxels in the internal layout  [ceil(D/G)][H_t][W_t][G][{T,W}]  with G = 2 (fp32) or 4 (fp16)
+ * bins per 128-bit access. */
+size_t ggt_volume_bytes(const ggt_volume_desc* desc);
+/* Binds caller-owned device storage (>= ggt_volume_bytes, 256-B aligned) and uploads the bin tables
+ * (synchronous small copy).  The storage content is otherwise untouched: call ggt_volume_reset. */
+int ggt_volume_bind(ggt_ctx* ctx, const ggt_volume_desc* desc, void* dev_storage, size_t bytes,
+                    ggt_volume** out);
+int ggt_volume_unbind(ggt_ctx* ctx, ggt_volume* vol);
+/* T = 0, W = 0 everywhere. */
+int ggt_volume_reset(ggt_ctx* ctx, ggt_volume* vol, void* stream);
+/* Canonical export for tests: bin-fastest idx = (v*W_t + u)*D + j, separate fp32 T and W arrays. */
+int ggt_volume_export(ggt_ctx* ctx, const ggt_volume* vol, float* dev_T, float* dev_W, void* stream);
+/* Copies of the tables the kernels use (host out arrays of D floats; either may be NULL). */
+int ggt_volume_tables(const ggt_volume* vol, float* host_z, float* host_tau);
+
+/* ---- step a1-a2: temporal depth refinement of one input view (Eq. 1-2) ----------- */
+/* dev_rgb_cur / dev_rgb_prev: uint8, height x width pixels of rgb_pixel_stride (3 or 4) bytes, channels
+ * 0..2 = RGB.  dev_rgb_prev == NULL -> first frame: M = 1, state = depth_cur.
+ * dev_depth_state: in = refined depth of frame t-1, out = refined depth of frame t (in place).
+ * dev_mask_out (optional): fp32 height x width soft mask M.  dev_pooled_out (optional): uint16
+ * ceil(H/4) x ceil(W/4) max-pooled block L1 colour difference (integer, exact). */
+int ggt_refine_depth(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t* dev_rgb_cur,
+                     const uint8_t* dev_rgb_prev, int32_t rgb_pixel_stride, const float* dev_depth_cur,
+                     float* dev_depth_state, float* dev_mask_out, uint16_t* dev_pooled_out,
+                     const ggt_refine_params* params, void* stream);
+
+/* ---- steps a3-a6: fuse V depth maps into the target-view TSDF ----------------- */
+/* target, views: HOST.  dev_depths: HOST array of n_views DEVICE pointers to fp32 height x width
+ * z-depth maps of the corresponding view (<= 0 invalid).  1 <= n_views <= GGT_MAX_VIEWS.
+ * target->width/height must equal the volume's.  flags: GGT_OVERWRITE or GGT_ACCUMULATE. */
+int ggt_integrate(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
+                  const ggt_camera* views, const float* const* dev_depths, uint32_t flags, void* stream);
+
+/* ---- step a7: zero-crossing depth (reading P13) ------------------------------------- */
+/* Outputs are fp32 / int32 H_t x W_t; any may be NULL.  Miss: depth 0, conf 0, bin -1. */
+int ggt_extract_depth(ggt_ctx* ctx, const ggt_volume* vol, float* dev_depth, float* dev_conf,
+                      int32_t* dev_bin, void* stream);
+
+/* ---- fused a3-a7: ggt_integrate that also emits what ggt_extract_depth would, in the same pass ---- */
+/* Same volume result as ggt_integrate followed by ggt_extract_depth, without re-reading the volume. */
+int ggt_integrate_extract(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
+                          const ggt_camera* views, const float* const* dev_depths, uint32_t flags,
+                          float* dev_depth, float* dev_conf, int32_t* dev_bin, void* stream);
+
+/* ---- end-to-end frame from HOST buffers (bench.py "e2e") ----------------------------------------- */
+/* One whole frame through the three steps with host<->device copies inside the call, all enqueued on
+ * `stream` without synchronising.  All n_views views must have the same width x height.
+ *   host_rgb_cur[k]   uint8 HxWx3 colour of view k at this frame (host; array or entry may be NULL -> that
+ *                     view is not refined, its depth is used as is); params NULL also disables refinement.
+ *   host_depth_cur[k] fp32 HxW z-depth of view k (host).
+ *   slots[k]          which history slot (0 <= slot < n_slots, e.g. the rig camera index) view k uses: the
+ *                     slot keeps the previous colour image and the refined-depth state in `dev_staging`.
+ *   host_slot_state   n_slots words, in/out, zero-initialised by the caller before the first frame
+ *                     (bit 0: slot has history, bit 1: ping-pong parity).  A slot without history gets the
+ *                     first-frame rule (M = 1).
+ *   dev_staging       caller-owned device memory, >= ggt_frame_staging_bytes, 256-B aligned.
+ *   host_depth / host_conf  fp32 H_t x W_t results (host; either may be NULL). */
+size_t ggt_frame_staging_bytes(const ggt_volume_desc* desc, int32_t n_slots, int32_t n_views, int32_t width,
+                               int32_t height);
+int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
+                   const ggt_camera* views, const uint8_t* const* host_rgb_cur, const float* const* host_depth_cur,
+                   const int32_t* slots, int32_t n_slots, uint32_t* host_slot_state,
+                   const ggt_refine_params* params, uint32_t flags, void* dev_staging, size_t staging_bytes,
+                   float* host_depth, float* host_conf, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GGT_H_ */

@@ -1,0 +1,274 @@
+"""Thin ctypes binding of the C ABI in include/ggt.h — argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libggt.so; torch is used for device memory and
+streams.  There is no fallback: if the library is missing or there is no CUDA device, calls raise.
+Function names mirror the C entry points (ggt_refine_depth, ggt_integrate, ggt_extract_depth, ...).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import List, Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libggt.so")
+
+GGT_OK = 0
+GGT_F32, GGT_F16 = 0, 1
+GGT_OVERWRITE, GGT_ACCUMULATE = 0, 1
+GGT_MAX_VIEWS = 16
+
+EXPORTS = [
+    "ggt_create", "ggt_destroy", "ggt_last_error", "ggt_launch_count", "ggt_workspace_bytes", "ggt_set_workspace",
+    "ggt_volume_bytes", "ggt_volume_bind", "ggt_volume_unbind", "ggt_volume_reset", "ggt_volume_export",
+    "ggt_volume_tables", "ggt_refine_depth", "ggt_integrate", "ggt_extract_depth", "ggt_integrate_extract",
+    "ggt_frame_staging_bytes", "ggt_frame_host",
+]
+
+
+class GgtError(RuntimeError):
+    pass
+
+
+class ggt_camera(ctypes.Structure):
+    _fields_ = [("fx", ctypes.c_float), ("fy", ctypes.c_float), ("cx", ctypes.c_float), ("cy", ctypes.c_float),
+                ("R", ctypes.c_float * 9), ("t", ctypes.c_float * 3),
+                ("width", ctypes.c_int32), ("height", ctypes.c_int32)]
+
+
+class ggt_refine_params(ctypes.Structure):
+    _fields_ = [("lambda_t", ctypes.c_float), ("beta", ctypes.c_float), ("theta", ctypes.c_float),
+                ("downscale", ctypes.c_int32), ("pool", ctypes.c_int32)]
+
+
+class ggt_volume_desc(ctypes.Structure):
+    _fields_ = [("width", ctypes.c_int32), ("height", ctypes.c_int32), ("bins", ctypes.c_int32),
+                ("z_bins", ctypes.POINTER(ctypes.c_float)), ("trunc_bins", ctypes.c_float),
+                ("trunc_metric", ctypes.c_float), ("w_sigma0", ctypes.c_float), ("w_clip", ctypes.c_float),
+                ("w_window", ctypes.c_int32), ("weight_cap", ctypes.c_float), ("decay", ctypes.c_float),
+                ("dtype", ctypes.c_int32)]
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen libggt.so (built in-tree by paper_2505_18932_b200/build.py) and declare signatures."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise GgtError("libggt.so not found at %s: run `python -m paper_2505_18932_b200.build` "
+                       "(there is no CPU fallback)" % LIB_PATH)
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i32, u32, f32p = ctypes.c_void_p, ctypes.c_int32, ctypes.c_uint32, ctypes.POINTER(ctypes.c_float)
+    camp, descp = ctypes.POINTER(ggt_camera), ctypes.POINTER(ggt_volume_desc)
+    lib.ggt_create.argtypes = [ctypes.POINTER(vp)]
+    lib.ggt_destroy.argtypes = [vp]
+    lib.ggt_last_error.argtypes = [vp]
+    lib.ggt_last_error.restype = ctypes.c_char_p
+    lib.ggt_launch_count.argtypes = [vp]
+    lib.ggt_launch_count.restype = ctypes.c_int64
+    lib.ggt_workspace_bytes.argtypes = [i32, i32, i32]
+    lib.ggt_workspace_bytes.restype = ctypes.c_size_t
+    lib.ggt_set_workspace.argtypes = [vp, vp, ctypes.c_size_t]
+    lib.ggt_volume_bytes.argtypes = [descp]
+    lib.ggt_volume_bytes.restype = ctypes.c_size_t
+    lib.ggt_volume_bind.argtypes = [vp, descp, vp, ctypes.c_size_t, ctypes.POINTER(vp)]
+    lib.ggt_volume_unbind.argtypes = [vp, vp]
+    lib.ggt_volume_reset.argtypes = [vp, vp, vp]
+    lib.ggt_volume_export.argtypes = [vp, vp, vp, vp, vp]
+    lib.ggt_volume_tables.argtypes = [vp, f32p, f32p]
+    lib.ggt_refine_depth.argtypes = [vp, i32, i32, vp, vp, i32, vp, vp, vp, vp, ctypes.POINTER(ggt_refine_params), vp]
+    lib.ggt_integrate.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), u32, vp]
+    lib.ggt_extract_depth.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.ggt_integrate_extract.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), u32, vp, vp, vp, vp]
+    lib.ggt_frame_staging_bytes.argtypes = [descp, i32, i32, i32, i32]
+    lib.ggt_frame_staging_bytes.restype = ctypes.c_size_t
+    lib.ggt_frame_host.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), ctypes.POINTER(vp),
+                                   ctypes.POINTER(i32), i32, ctypes.POINTER(u32),
+                                   ctypes.POINTER(ggt_refine_params), u32, vp, ctypes.c_size_t, vp, vp, vp]
+    _lib = lib
+    return lib
+
+
+def to_camera(c) -> ggt_camera:
+    """Marshal any object with fx, fy, cx, cy, R (3x3), t (3), width, height."""
+    o = ggt_camera()
+    o.fx, o.fy, o.cx, o.cy = float(c.fx), float(c.fy), float(c.cx), float(c.cy)
+    o.R[:] = [float(x) for x in np.asarray(c.R, dtype=np.float32).reshape(9)]
+    o.t[:] = [float(x) for x in np.asarray(c.t, dtype=np.float32).reshape(3)]
+    o.width, o.height = int(c.width), int(c.height)
+    return o
+
+
+def _ptr(t) -> Optional[int]:
+    return None if t is None else t.data_ptr()
+
+
+def _stream() -> int:
+    import torch
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _refine_params(lambda_t=0.7, beta=0.6, theta=0.0, downscale=4, pool=3) -> ggt_refine_params:
+    return ggt_refine_params(lambda_t, beta, theta, downscale, pool)
+
+
+class Context:
+    """ggt_ctx: one per (device, stream of use).  Owns no frame state."""
+
+    def __init__(self):
+        import torch
+        if not torch.cuda.is_available():
+            raise GgtError("no CUDA device: the ggt library has no CPU path")
+        self.lib = load_library()
+        h = ctypes.c_void_p()
+        rc = self.lib.ggt_create(ctypes.byref(h))
+        if rc != GGT_OK:
+            raise GgtError("ggt_create: %s" % self.lib.ggt_last_error(None).decode())
+        self.h = h
+        self._ws = None
+
+    def check(self, rc: int, what: str):
+        if rc != GGT_OK:
+            raise GgtError("%s failed (%d): %s" % (what, rc, self.lib.ggt_last_error(self.h).decode()))
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.ggt_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def launch_count(self) -> int:
+        return int(self.lib.ggt_launch_count(self.h))
+
+    def ggt_set_workspace(self, n_views: int, width: int, height: int):
+        import torch
+        n = self.lib.ggt_workspace_bytes(n_views, width, height)
+        self._ws = torch.empty(n, dtype=torch.uint8, device="cuda")
+        self.check(self.lib.ggt_set_workspace(self.h, self._ws.data_ptr(), n), "ggt_set_workspace")
+
+    # ---- a1-a2 -------------------------------------------------------------------------------------
+    def ggt_refine_depth(self, rgb_cur, rgb_prev, depth_cur, depth_state, mask_out=None, pooled_out=None,
+                         lambda_t=0.7, beta=0.6, theta=0.0, downscale=4, pool=3):
+        """In-place update of `depth_state` (torch fp32 HxW, cuda).  rgb_*: torch uint8 HxWx{3,4} or None."""
+        H, W = depth_cur.shape
+        stride = 3 if rgb_cur is None else int(rgb_cur.shape[2])
+        for t in (rgb_cur, rgb_prev, depth_cur, depth_state, mask_out, pooled_out):
+            assert t is None or (t.is_cuda and t.is_contiguous())
+        prm = _refine_params(lambda_t, beta, theta, downscale, pool)
+        rc = self.lib.ggt_refine_depth(self.h, W, H, _ptr(rgb_cur), _ptr(rgb_prev), stride, _ptr(depth_cur),
+                                       _ptr(depth_state), _ptr(mask_out), _ptr(pooled_out), ctypes.byref(prm),
+                                       _stream())
+        self.check(rc, "ggt_refine_depth")
+
+    # ---- volume ------------------------------------------------------------------------------------
+    def ggt_volume_bind(self, width, height, z_bins, dtype=GGT_F32, trunc_bins=2.0, trunc_metric=0.0,
+                        w_sigma0=0.001, w_clip=0.02, w_window=7, weight_cap=64.0, decay=1.0) -> "Volume":
+        return Volume(self, width, height, z_bins, dtype, trunc_bins, trunc_metric, w_sigma0, w_clip, w_window,
+                      weight_cap, decay)
+
+    # ---- a3-a6 -------------------------------------------------------------------------------------
+    def _cams(self, target, views):
+        V = len(views)
+        arr = (ggt_camera * V)(*[to_camera(c) for c in views])
+        return to_camera(target), arr
+
+    def ggt_integrate(self, vol: "Volume", target, views: Sequence, depths: Sequence, flags=GGT_OVERWRITE):
+        V = len(views)
+        t, arr = self._cams(target, views)
+        for d in depths:
+            assert d.is_cuda and d.is_contiguous() and d.dtype.is_floating_point
+        ptrs = (ctypes.c_void_p * V)(*[d.data_ptr() for d in depths])
+        rc = self.lib.ggt_integrate(self.h, vol.h, ctypes.byref(t), V, arr, ptrs, flags, _stream())
+        self.check(rc, "ggt_integrate")
+
+    def ggt_integrate_extract(self, vol: "Volume", target, views, depths, flags=GGT_OVERWRITE, depth=None,
+                              conf=None, bins=None):
+        V = len(views)
+        t, arr = self._cams(target, views)
+        ptrs = (ctypes.c_void_p * V)(*[d.data_ptr() for d in depths])
+        rc = self.lib.ggt_integrate_extract(self.h, vol.h, ctypes.byref(t), V, arr, ptrs, flags, _ptr(depth),
+                                            _ptr(conf), _ptr(bins), _stream())
+        self.check(rc, "ggt_integrate_extract")
+
+    # ---- a7 ----------------------------------------------------------------------------------------
+    def ggt_extract_depth(self, vol: "Volume", depth=None, conf=None, bins=None):
+        rc = self.lib.ggt_extract_depth(self.h, vol.h, _ptr(depth), _ptr(conf), _ptr(bins), _stream())
+        self.check(rc, "ggt_extract_depth")
+
+    # ---- end-to-end from host buffers -----------------------------------------------------------------
+    def ggt_frame_host(self, vol: "Volume", target, views, host_rgb: Optional[Sequence], host_depth_in: Sequence,
+                       slots: Sequence[int], slot_state: np.ndarray, staging, host_depth, host_conf,
+                       flags=GGT_OVERWRITE, refine_params: Optional[ggt_refine_params] = None):
+        """host_* are pinned CPU torch tensors; slot_state is a numpy uint32 array kept by the caller."""
+        V = len(views)
+        t, arr = self._cams(target, views)
+        rgbp = None
+        if host_rgb is not None:
+            rgbp = (ctypes.c_void_p * V)(*[None if r is None else r.data_ptr() for r in host_rgb])
+        dp = (ctypes.c_void_p * V)(*[d.data_ptr() for d in host_depth_in])
+        sl = (ctypes.c_int32 * V)(*[int(s) for s in slots])
+        rc = self.lib.ggt_frame_host(
+            self.h, vol.h, ctypes.byref(t), V, arr, rgbp, dp, sl, int(slot_state.size),
+            slot_state.ctypes.data_as(ctypes.POINTER(ctypes.c_uint32)),
+            ctypes.byref(refine_params) if refine_params is not None else None, flags, staging.data_ptr(),
+            staging.numel(), _ptr(host_depth), _ptr(host_conf), _stream())
+        self.check(rc, "ggt_frame_host")
+
+
+class Volume:
+    """ggt_volume bound to a torch-owned uint8 storage tensor."""
+
+    def __init__(self, ctx: Context, width, height, z_bins, dtype, trunc_bins, trunc_metric, w_sigma0, w_clip,
+                 w_window, weight_cap, decay):
+        import torch
+        self.ctx = ctx
+        self.z = np.ascontiguousarray(z_bins, dtype=np.float32)
+        self.desc = ggt_volume_desc(int(width), int(height), int(self.z.size),
+                                    self.z.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), trunc_bins, trunc_metric,
+                                    w_sigma0, w_clip, int(w_window), weight_cap, decay, int(dtype))
+        self.width, self.height, self.bins, self.dtype = int(width), int(height), int(self.z.size), int(dtype)
+        n = ctx.lib.ggt_volume_bytes(ctypes.byref(self.desc))
+        if n == 0:
+            raise GgtError("ggt_volume_bytes: bad descriptor")
+        self.nbytes = int(n)
+        self.storage = torch.empty(n, dtype=torch.uint8, device="cuda")
+        h = ctypes.c_void_p()
+        ctx.check(ctx.lib.ggt_volume_bind(ctx.h, ctypes.byref(self.desc), self.storage.data_ptr(), n, ctypes.byref(h)),
+                  "ggt_volume_bind")
+        self.h = h
+
+    def ggt_volume_reset(self):
+        self.ctx.check(self.ctx.lib.ggt_volume_reset(self.ctx.h, self.h, _stream()), "ggt_volume_reset")
+
+    def ggt_volume_export(self):
+        """(T, W) torch fp32 tensors of shape (H_t*W_t, D), canonical bin-fastest layout."""
+        import torch
+        n = self.width * self.height
+        T = torch.empty((n, self.bins), dtype=torch.float32, device="cuda")
+        W = torch.empty((n, self.bins), dtype=torch.float32, device="cuda")
+        self.ctx.check(self.ctx.lib.ggt_volume_export(self.ctx.h, self.h, T.data_ptr(), W.data_ptr(), _stream()),
+                       "ggt_volume_export")
+        return T, W
+
+    def ggt_volume_tables(self):
+        z = np.empty(self.bins, np.float32)
+        tau = np.empty(self.bins, np.float32)
+        self.ctx.lib.ggt_volume_tables(self.h, z.ctypes.data_as(ctypes.POINTER(ctypes.c_float)),
+                                       tau.ctypes.data_as(ctypes.POINTER(ctypes.c_float)))
+        return z, tau
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.ctx.lib.ggt_volume_unbind(self.ctx.h, self.h)
+            self.h = None

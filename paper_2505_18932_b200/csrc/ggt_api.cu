@@ -1,0 +1,413 @@
+// ggt_api.cu — the C ABI declared in include/ggt.h: argument validation, host-side camera algebra,
+// workspace handling and kernel launches.  No compute happens on the host beyond the 12 floats per view of
+// the relative transform and the bin tables; there is no CPU fallback.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "ggt_internal.h"
+
+namespace {
+
+std::string g_create_error;
+
+int fail(ggt_ctx* ctx, int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (ctx) ctx->err = buf; else g_create_error = buf;
+    return code;
+}
+
+int cuda_fail(ggt_ctx* ctx, cudaError_t e, const char* what) {
+    return fail(ctx, GGT_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// Relative transform of PAPER.md:331 in double, rounded once to float:
+//   p_world = R_t^T (z K_t^{-1} (uc, vc, 1)^T - t_t);  (x, y, w) = K_k (R_k p_world + t_k)
+//   => (x, y, w) = z * Hm (uc, vc, 1)^T + e  with  Hm = K_k R_k R_t^T K_t^{-1},  e = K_k (t_k - R_k R_t^T t_t).
+// Products are plain left-to-right 3-term sums (DESIGN.md fixes the order so that two independent
+// implementations round identically).
+void relative_transform(const ggt_camera& tg, const ggt_camera& vw, float* h, float* e) {
+    double RkRtT[9];
+    for (int r = 0; r < 3; ++r)
+        for (int c = 0; c < 3; ++c)
+            RkRtT[3 * r + c] = (double)vw.R[3 * r] * (double)tg.R[3 * c] + (double)vw.R[3 * r + 1] * (double)tg.R[3 * c + 1] +
+                               (double)vw.R[3 * r + 2] * (double)tg.R[3 * c + 2];
+    const double K[9] = {vw.fx, 0.0, vw.cx, 0.0, vw.fy, vw.cy, 0.0, 0.0, 1.0};
+    const double fx = tg.fx, fy = tg.fy, cx = tg.cx, cy = tg.cy;
+    const double Ki[9] = {1.0 / fx, 0.0, -cx / fx, 0.0, 1.0 / fy, -cy / fy, 0.0, 0.0, 1.0};
+    double KR[9], Hm[9];
+    for (int r = 0; r < 3; ++r)
+        for (int c = 0; c < 3; ++c)
+            KR[3 * r + c] = K[3 * r] * RkRtT[c] + K[3 * r + 1] * RkRtT[3 + c] + K[3 * r + 2] * RkRtT[6 + c];
+    for (int r = 0; r < 3; ++r)
+        for (int c = 0; c < 3; ++c)
+            Hm[3 * r + c] = KR[3 * r] * Ki[c] + KR[3 * r + 1] * Ki[3 + c] + KR[3 * r + 2] * Ki[6 + c];
+    double d[3];
+    for (int r = 0; r < 3; ++r)
+        d[r] = (double)vw.t[r] - (RkRtT[3 * r] * (double)tg.t[0] + RkRtT[3 * r + 1] * (double)tg.t[1] +
+                                  RkRtT[3 * r + 2] * (double)tg.t[2]);
+    for (int r = 0; r < 3; ++r) e[r] = (float)(K[3 * r] * d[0] + K[3 * r + 1] * d[1] + K[3 * r + 2] * d[2]);
+    for (int i = 0; i < 9; ++i) h[i] = (float)Hm[i];
+}
+
+int check_desc(ggt_ctx* ctx, const ggt_volume_desc* d) {
+    if (!d) return fail(ctx, GGT_ERR_INVALID_ARG, "volume descriptor is NULL");
+    if (d->width <= 0 || d->height <= 0) return fail(ctx, GGT_ERR_SHAPE, "volume size %dx%d", d->width, d->height);
+    if (d->width > (1 << 20) || d->height > (1 << 20)) return fail(ctx, GGT_ERR_SHAPE, "volume too large");
+    if (d->bins < 2 || d->bins > GGT_MAX_BINS) return fail(ctx, GGT_ERR_SHAPE, "bins %d not in [2, %d]", d->bins, GGT_MAX_BINS);
+    if (d->dtype != GGT_F32 && d->dtype != GGT_F16) return fail(ctx, GGT_ERR_UNSUPPORTED, "dtype %d", d->dtype);
+    if (d->w_window != 0 && d->w_window != 7) return fail(ctx, GGT_ERR_UNSUPPORTED, "w_window %d (0 or 7)", d->w_window);
+    return GGT_OK;
+}
+
+size_t header_bytes_of(const ggt_volume_desc* d) {
+    const int G = ggt_group_of(d->dtype);
+    const int ng = (d->bins + G - 1) / G;
+    return align_up((size_t)2 * ng * G * sizeof(float), 256);
+}
+
+size_t voxel_bytes_of(const ggt_volume_desc* d) {
+    const int G = ggt_group_of(d->dtype);
+    const int ng = (d->bins + G - 1) / G;
+    return (size_t)ng * d->width * d->height * 16;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ggt_create(ggt_ctx** out) {
+    if (!out) return fail(nullptr, GGT_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n == 0) {
+        cudaGetLastError();
+        return fail(nullptr, GGT_ERR_CUDA, "no CUDA device (%s): the ggt library has no CPU path",
+                    e != cudaSuccess ? cudaGetErrorString(e) : "device count 0");
+    }
+    ggt_ctx* c = new (std::nothrow) ggt_ctx();
+    if (!c) return fail(nullptr, GGT_ERR_INVALID_ARG, "out of host memory");
+    cudaGetDevice(&c->device);
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device);
+    int major = 0;
+    cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, c->device);
+    if (major != 10) {
+        delete c;
+        return fail(nullptr, GGT_ERR_UNSUPPORTED, "device compute capability %d.x: this library is built for sm_100a only", major);
+    }
+    *out = c;
+    return GGT_OK;
+}
+
+int ggt_destroy(ggt_ctx* ctx) {
+    if (!ctx) return GGT_OK;
+    ggt_ctx* c = ctx;
+    if (c->ws_owned && c->ws) cudaFree(c->ws);
+    if (c->cq) cudaFree(c->cq);
+    delete c;
+    return GGT_OK;
+}
+
+const char* ggt_last_error(const ggt_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+int64_t ggt_launch_count(const ggt_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+size_t ggt_workspace_bytes(int32_t n_views, int32_t width, int32_t height) {
+    if (n_views <= 0 || width <= 0 || height <= 0) return 0;
+    return (size_t)n_views * align_up((size_t)width * height * sizeof(float2), 256);
+}
+
+int ggt_set_workspace(ggt_ctx* ctx, void* dev_workspace, size_t bytes) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    if (((uintptr_t)dev_workspace & 255) != 0) return fail(ctx, GGT_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    if (ctx->ws_owned && ctx->ws) cudaFree(ctx->ws);
+    ctx->ws = dev_workspace;
+    ctx->ws_bytes = dev_workspace ? bytes : 0;
+    ctx->ws_owned = false;
+    return GGT_OK;
+}
+
+size_t ggt_volume_bytes(const ggt_volume_desc* desc) {
+    if (!desc || desc->width <= 0 || desc->height <= 0 || desc->bins < 2) return 0;
+    return header_bytes_of(desc) + voxel_bytes_of(desc);
+}
+
+int ggt_volume_bind(ggt_ctx* ctx, const ggt_volume_desc* desc, void* dev_storage, size_t bytes, ggt_volume** out) {
+    if (!ctx || !out) return GGT_ERR_INVALID_ARG;
+    *out = nullptr;
+    int rc = check_desc(ctx, desc);
+    if (rc != GGT_OK) return rc;
+    if (!desc->z_bins) return fail(ctx, GGT_ERR_INVALID_ARG, "z_bins is NULL");
+    if (!dev_storage || ((uintptr_t)dev_storage & 255) != 0) return fail(ctx, GGT_ERR_INVALID_ARG, "storage NULL or not 256-byte aligned");
+    if (bytes < ggt_volume_bytes(desc)) return fail(ctx, GGT_ERR_SHAPE, "storage %zu B < required %zu B", bytes, ggt_volume_bytes(desc));
+    for (int j = 0; j < desc->bins; ++j) {
+        if (!(desc->z_bins[j] > 0.0f) || (j > 0 && !(desc->z_bins[j] > desc->z_bins[j - 1])))
+            return fail(ctx, GGT_ERR_INVALID_ARG, "z_bins must be positive and strictly increasing (bin %d)", j);
+    }
+    if (!(desc->trunc_metric > 0.0f) && !(desc->trunc_bins > 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "no truncation distance given");
+    ggt_volume* v = new (std::nothrow) ggt_volume();
+    if (!v) return fail(ctx, GGT_ERR_INVALID_ARG, "out of host memory");
+    v->desc = *desc;
+    const int D = desc->bins;
+    v->z.assign(desc->z_bins, desc->z_bins + D);
+    v->desc.z_bins = v->z.data();
+    v->tau.resize(D);
+    // tau_j = trunc_bins x local spacing, one-sided at the ends (reading P3), in double then float
+    for (int j = 0; j < D; ++j) {
+        double sp;
+        if (j == 0) sp = (double)v->z[1] - (double)v->z[0];
+        else if (j == D - 1) sp = (double)v->z[D - 1] - (double)v->z[D - 2];
+        else sp = ((double)v->z[j + 1] - (double)v->z[j - 1]) / 2.0;
+        v->tau[j] = desc->trunc_metric > 0.0f ? desc->trunc_metric : (float)((double)desc->trunc_bins * sp);
+    }
+    v->group = ggt_group_of(desc->dtype);
+    v->n_groups = (D + v->group - 1) / v->group;
+    v->header_bytes = header_bytes_of(desc);
+    v->voxel_bytes = voxel_bytes_of(desc);
+    v->dev_tables = static_cast<float*>(dev_storage);
+    v->dev_voxels = static_cast<char*>(dev_storage) + v->header_bytes;
+    const int Dpad = v->n_groups * v->group;
+    std::vector<float> tab(2 * (size_t)Dpad);
+    for (int j = 0; j < Dpad; ++j) {
+        tab[j] = v->z[j < D ? j : D - 1];
+        tab[Dpad + j] = v->tau[j < D ? j : D - 1];
+    }
+    cudaError_t e = cudaMemcpy(v->dev_tables, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { delete v; return cuda_fail(ctx, e, "upload of bin tables"); }
+    *out = v;
+    return GGT_OK;
+}
+
+int ggt_volume_unbind(ggt_ctx*, ggt_volume* vol) {
+    delete vol;
+    return GGT_OK;
+}
+
+int ggt_volume_reset(ggt_ctx* ctx, ggt_volume* vol, void* stream) {
+    if (!ctx || !vol) return GGT_ERR_INVALID_ARG;
+    cudaError_t e = cudaMemsetAsync(vol->dev_voxels, 0, vol->voxel_bytes, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "volume reset");
+    ctx->launches += 1;
+    return GGT_OK;
+}
+
+static GgtExtractParams extract_params(const ggt_volume* vol) {
+    GgtExtractParams p;
+    p.Wt = vol->desc.width; p.Ht = vol->desc.height; p.D = vol->desc.bins; p.n_groups = vol->n_groups;
+    p.tables = vol->dev_tables; p.voxels = vol->dev_voxels;
+    p.depth = nullptr; p.conf = nullptr; p.bin = nullptr;
+    return p;
+}
+
+int ggt_volume_export(ggt_ctx* ctx, const ggt_volume* vol, float* dev_T, float* dev_W, void* stream) {
+    if (!ctx || !vol || !dev_T || !dev_W) return GGT_ERR_INVALID_ARG;
+    cudaError_t e = ggt_launch_export(extract_params(vol), vol->desc.dtype, dev_T, dev_W, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "volume export");
+    ctx->launches += 1;
+    return GGT_OK;
+}
+
+int ggt_volume_tables(const ggt_volume* vol, float* host_z, float* host_tau) {
+    if (!vol) return GGT_ERR_INVALID_ARG;
+    if (host_z) memcpy(host_z, vol->z.data(), vol->z.size() * sizeof(float));
+    if (host_tau) memcpy(host_tau, vol->tau.data(), vol->tau.size() * sizeof(float));
+    return GGT_OK;
+}
+
+int ggt_refine_depth(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t* dev_rgb_cur,
+                     const uint8_t* dev_rgb_prev, int32_t rgb_pixel_stride, const float* dev_depth_cur,
+                     float* dev_depth_state, float* dev_mask_out, uint16_t* dev_pooled_out,
+                     const ggt_refine_params* params, void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    ggt_ctx* c = ctx;
+    if (width <= 0 || height <= 0) return fail(ctx, GGT_ERR_SHAPE, "image size %dx%d", width, height);
+    if (!dev_depth_cur || !dev_depth_state || !params) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL depth / params pointer");
+    if (dev_rgb_prev && !dev_rgb_cur) return fail(ctx, GGT_ERR_INVALID_ARG, "rgb_prev given without rgb_cur");
+    if (rgb_pixel_stride != 3 && rgb_pixel_stride != 4) return fail(ctx, GGT_ERR_INVALID_ARG, "rgb_pixel_stride %d (3 or 4)", rgb_pixel_stride);
+    if (params->downscale != 4 || params->pool != 3) return fail(ctx, GGT_ERR_UNSUPPORTED, "only downscale 4 / pool 3 (PAPER.md:81) are implemented");
+    if (!(params->lambda_t > 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "lambda_t must be > 0");
+    if (dev_rgb_prev) {
+        const size_t need = (size_t)((width + 3) / 4) * ((height + 3) / 4) * sizeof(uint16_t);
+        if (c->cq_bytes < need) {
+            if (c->cq) cudaFree(c->cq);
+            c->cq = nullptr; c->cq_bytes = 0;
+            cudaError_t e = cudaMalloc(&c->cq, need);
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "scratch for block differences");
+            c->cq_bytes = need;
+        }
+    }
+    int n = 0;
+    cudaError_t e = ggt_launch_refine(width, height, dev_rgb_cur, dev_rgb_prev, rgb_pixel_stride, dev_depth_cur,
+                                      dev_depth_state, dev_mask_out, dev_pooled_out, c->cq, params->lambda_t,
+                                      params->beta, params->theta, (cudaStream_t)stream, &n);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "ggt_refine_depth launch");
+    ctx->launches += n;
+    return GGT_OK;
+}
+
+// Shared front end of ggt_integrate / ggt_integrate_extract: validation, workspace, weight maps, launch.
+static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
+                          const ggt_camera* views, const float* const* dev_depths, uint32_t flags, bool fused,
+                          float* dev_depth, float* dev_conf, int32_t* dev_bin, void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    if (!vol || !target || !views || !dev_depths) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL volume / camera / depth pointer");
+    if (n_views < 1 || n_views > GGT_MAX_VIEWS) return fail(ctx, GGT_ERR_SHAPE, "n_views %d not in [1, %d]", n_views, GGT_MAX_VIEWS);
+    if (flags != GGT_OVERWRITE && flags != GGT_ACCUMULATE) return fail(ctx, GGT_ERR_INVALID_ARG, "flags %u", flags);
+    if (target->width != vol->desc.width || target->height != vol->desc.height)
+        return fail(ctx, GGT_ERR_SHAPE, "target %dx%d does not match the volume %dx%d", target->width, target->height,
+                    vol->desc.width, vol->desc.height);
+    if (!(target->fx > 0.0f) || !(target->fy > 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "target focal length");
+    size_t need = 0;
+    for (int k = 0; k < n_views; ++k) {
+        if (views[k].width <= 0 || views[k].height <= 0 || views[k].width > (1 << 20) || views[k].height > (1 << 20))
+            return fail(ctx, GGT_ERR_SHAPE, "view %d size %dx%d", k, views[k].width, views[k].height);
+        if (!dev_depths[k]) return fail(ctx, GGT_ERR_INVALID_ARG, "dev_depths[%d] is NULL", k);
+        need += align_up((size_t)views[k].width * views[k].height * sizeof(float2), 256);
+    }
+    if (ctx->ws_bytes < need) {
+        if (ctx->ws && !ctx->ws_owned) return fail(ctx, GGT_ERR_SHAPE, "workspace %zu B < required %zu B", ctx->ws_bytes, need);
+        if (ctx->ws) cudaFree(ctx->ws);   // synchronises: only between frames, when the view set grows
+        ctx->ws = nullptr; ctx->ws_bytes = 0;
+        cudaError_t e = cudaMalloc(&ctx->ws, need);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "workspace allocation");
+        ctx->ws_bytes = need; ctx->ws_owned = true;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    GgtIntegrateParams p;
+    memset(&p, 0, sizeof p);
+    p.Wt = vol->desc.width; p.Ht = vol->desc.height; p.D = vol->desc.bins;
+    p.n_views = n_views; p.n_groups = vol->n_groups;
+    p.accumulate = flags == GGT_ACCUMULATE ? 1 : 0;
+    p.decay = vol->desc.decay; p.cap = vol->desc.weight_cap;
+    p.tables = vol->dev_tables; p.voxels = vol->dev_voxels;
+    p.depth = dev_depth; p.conf = dev_conf; p.bin = dev_bin;
+    char* w = static_cast<char*>(ctx->ws);
+    for (int k = 0; k < n_views; ++k) {
+        relative_transform(*target, views[k], p.v[k].h, p.v[k].e);
+        p.v[k].map = reinterpret_cast<const float2*>(w);
+        p.v[k].width = views[k].width; p.v[k].height = views[k].height;
+        cudaError_t e = ggt_launch_weight_map(views[k].width, views[k].height, dev_depths[k], reinterpret_cast<float2*>(w),
+                                              vol->desc.w_sigma0, vol->desc.w_clip, vol->desc.w_window, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "weight-map launch");
+        ctx->launches += 1;
+        w += align_up((size_t)views[k].width * views[k].height * sizeof(float2), 256);
+    }
+    cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, fused, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "integrate launch");
+    ctx->launches += 1;
+    return GGT_OK;
+}
+
+int ggt_integrate(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
+                  const ggt_camera* views, const float* const* dev_depths, uint32_t flags, void* stream) {
+    return integrate_impl(ctx, vol, target, n_views, views, dev_depths, flags, false, nullptr, nullptr, nullptr, stream);
+}
+
+int ggt_integrate_extract(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
+                          const ggt_camera* views, const float* const* dev_depths, uint32_t flags,
+                          float* dev_depth, float* dev_conf, int32_t* dev_bin, void* stream) {
+    return integrate_impl(ctx, vol, target, n_views, views, dev_depths, flags, true, dev_depth, dev_conf, dev_bin, stream);
+}
+
+int ggt_extract_depth(ggt_ctx* ctx, const ggt_volume* vol, float* dev_depth, float* dev_conf, int32_t* dev_bin,
+                      void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    if (!vol) return fail(ctx, GGT_ERR_INVALID_ARG, "volume is NULL");
+    GgtExtractParams p = extract_params(vol);
+    p.depth = dev_depth; p.conf = dev_conf; p.bin = dev_bin;
+    cudaError_t e = ggt_launch_extract(p, vol->desc.dtype, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "extract launch");
+    ctx->launches += 1;
+    return GGT_OK;
+}
+
+// ---- end-to-end frame from host buffers -------------------------------------------------------------
+// staging layout (every block 256-B aligned), all views width x height:
+//   per slot s:  rgb[2][H*W*3] (ping-pong current / previous colour), state[H*W] fp32 refined depth
+//   per view k:  depth_cur[H*W] fp32
+//   outputs:     depth[Ht*Wt], conf[Ht*Wt] fp32
+size_t ggt_frame_staging_bytes(const ggt_volume_desc* desc, int32_t n_slots, int32_t n_views, int32_t width,
+                               int32_t height) {
+    if (!desc || n_slots <= 0 || n_views <= 0 || width <= 0 || height <= 0) return 0;
+    const size_t px = (size_t)width * height;
+    const size_t rgb = align_up(px * 3, 256), dep = align_up(px * 4, 256);
+    const size_t out = align_up((size_t)desc->width * desc->height * 4, 256);
+    return (size_t)n_slots * (2 * rgb + dep) + (size_t)n_views * dep + 2 * out;
+}
+
+int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
+                   const ggt_camera* views, const uint8_t* const* host_rgb_cur, const float* const* host_depth_cur,
+                   const int32_t* slots, int32_t n_slots, uint32_t* host_slot_state,
+                   const ggt_refine_params* params, uint32_t flags, void* dev_staging, size_t staging_bytes,
+                   float* host_depth, float* host_conf, void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    if (!vol || !target || !views || !host_depth_cur || !slots || !host_slot_state || !dev_staging)
+        return fail(ctx, GGT_ERR_INVALID_ARG, "NULL argument to ggt_frame_host");
+    if (n_views < 1 || n_views > GGT_MAX_VIEWS || n_slots < 1) return fail(ctx, GGT_ERR_SHAPE, "n_views / n_slots");
+    const int W = views[0].width, H = views[0].height;
+    for (int k = 0; k < n_views; ++k) {
+        if (views[k].width != W || views[k].height != H) return fail(ctx, GGT_ERR_SHAPE, "ggt_frame_host needs equal view sizes");
+        if (slots[k] < 0 || slots[k] >= n_slots) return fail(ctx, GGT_ERR_INVALID_ARG, "slots[%d] = %d", k, slots[k]);
+        if (!host_depth_cur[k]) return fail(ctx, GGT_ERR_INVALID_ARG, "host_depth_cur[%d] is NULL", k);
+    }
+    if (((uintptr_t)dev_staging & 255) != 0) return fail(ctx, GGT_ERR_INVALID_ARG, "staging must be 256-byte aligned");
+    const size_t need = ggt_frame_staging_bytes(&vol->desc, n_slots, n_views, W, H);
+    if (staging_bytes < need) return fail(ctx, GGT_ERR_SHAPE, "staging %zu B < required %zu B", staging_bytes, need);
+    const bool refine = host_rgb_cur != nullptr && params != nullptr;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t px = (size_t)W * H;
+    const size_t rgb = align_up(px * 3, 256), dep = align_up(px * 4, 256);
+    const size_t out = align_up((size_t)vol->desc.width * vol->desc.height * 4, 256);
+    char* base = static_cast<char*>(dev_staging);
+    char* view_base = base + (size_t)n_slots * (2 * rgb + dep);
+    char* out_base = view_base + (size_t)n_views * dep;
+    const float* dptr[GGT_MAX_VIEWS];
+    for (int k = 0; k < n_views; ++k) {
+        char* slot = base + (size_t)slots[k] * (2 * rgb + dep);
+        float* state = reinterpret_cast<float*>(slot + 2 * rgb);
+        float* dcur = reinterpret_cast<float*>(view_base + (size_t)k * dep);
+        cudaError_t e = cudaMemcpyAsync(dcur, host_depth_cur[k], px * 4, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D depth");
+        if (refine && host_rgb_cur[k]) {
+            uint32_t& s = host_slot_state[slots[k]];          // bit 0: has history, bit 1: parity of "current"
+            const int cur = (s >> 1) & 1 ? 0 : 1;
+            uint8_t* rc = reinterpret_cast<uint8_t*>(slot + (size_t)cur * rgb);
+            const uint8_t* rp = (s & 1) ? reinterpret_cast<const uint8_t*>(slot + (size_t)(1 - cur) * rgb) : nullptr;
+            e = cudaMemcpyAsync(rc, host_rgb_cur[k], px * 3, cudaMemcpyHostToDevice, st);
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D colour");
+            int rcode = ggt_refine_depth(ctx, W, H, rc, rp, 3, dcur, state, nullptr, nullptr, params, stream);
+            if (rcode != GGT_OK) return rcode;
+            s = 1u | ((uint32_t)cur << 1);
+            dptr[k] = state;
+        } else {
+            dptr[k] = dcur;
+        }
+    }
+    float* d_depth = reinterpret_cast<float*>(out_base);
+    float* d_conf = reinterpret_cast<float*>(out_base + out);
+    int rcode = ggt_integrate(ctx, vol, target, n_views, views, dptr, flags, stream);
+    if (rcode != GGT_OK) return rcode;
+    rcode = ggt_extract_depth(ctx, vol, host_depth ? d_depth : nullptr, host_conf ? d_conf : nullptr, nullptr, stream);
+    if (rcode != GGT_OK) return rcode;
+    const size_t ob = (size_t)vol->desc.width * vol->desc.height * 4;
+    if (host_depth) {
+        cudaError_t e = cudaMemcpyAsync(host_depth, d_depth, ob, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "D2H depth");
+    }
+    if (host_conf) {
+        cudaError_t e = cudaMemcpyAsync(host_conf, d_conf, ob, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "D2H confidence");
+    }
+    return GGT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,77 @@
+// ggt_internal.h — private declarations of the CUDA path (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/ggt.h"
+
+// ---- device-side parameter blocks (passed by value as __grid_constant__ kernel parameters) --------
+struct GgtViewParams {
+    float h[9];            // H_k = K_k R_k R_t^T K_t^{-1}   (row-major)
+    float e[3];            // e_k = K_k (t_k - R_k R_t^T t_t)
+    const float2* map;     // interleaved {depth, omega}, height x width
+    int32_t width, height;
+};
+
+struct GgtIntegrateParams {
+    int32_t Wt, Ht, D;     // target width / height, bins
+    int32_t n_views;
+    int32_t n_groups;      // ceil(D / G)
+    int32_t accumulate;    // 0 overwrite, 1 running average
+    float decay, cap;
+    const float* tables;   // device: z[0..Dpad) then tau[0..Dpad), Dpad = n_groups * G
+    void* voxels;          // device: [n_groups][Ht][Wt][G][{T,W}]
+    float* depth;          // fused extract outputs (may be null)
+    float* conf;
+    int32_t* bin;
+    GgtViewParams v[GGT_MAX_VIEWS];
+};
+
+struct GgtExtractParams {
+    int32_t Wt, Ht, D, n_groups;
+    const float* tables;
+    const void* voxels;
+    float* depth;
+    float* conf;
+    int32_t* bin;
+};
+
+// ---- host objects -----------------------------------------------------------------------------------
+struct ggt_ctx {
+    int device = 0;
+    int sm_count = 148;
+    std::string err;
+    int64_t launches = 0;
+    void* ws = nullptr;            // {depth, omega} maps scratch
+    size_t ws_bytes = 0;
+    bool ws_owned = false;
+    uint16_t* cq = nullptr;        // quarter-res block differences of ggt_refine_depth (context-owned)
+    size_t cq_bytes = 0;
+};
+
+struct ggt_volume {
+    ggt_volume_desc desc;
+    std::vector<float> z, tau;     // host copies of the tables (D entries)
+    int32_t group = 2;             // G: bins per 128-bit access
+    int32_t n_groups = 0;
+    size_t header_bytes = 0;
+    size_t voxel_bytes = 0;
+    float* dev_tables = nullptr;   // inside the caller's storage
+    void* dev_voxels = nullptr;    // inside the caller's storage
+};
+
+static inline int ggt_group_of(int dtype) { return dtype == GGT_F16 ? 4 : 2; }
+
+// ---- kernel launchers (each returns cudaError_t of the launch) ----------------------------------------
+cudaError_t ggt_launch_refine(int W, int H, const uint8_t* rgb_cur, const uint8_t* rgb_prev, int stride,
+                              const float* depth_cur, float* depth_state, float* mask_out,
+                              uint16_t* pooled_out, uint16_t* cq_scratch, float lambda_t, float beta,
+                              float theta, cudaStream_t st, int* n_launches);
+cudaError_t ggt_launch_weight_map(int W, int H, const float* depth, float2* out, float sigma0, float clip,
+                                  int window, cudaStream_t st);
+cudaError_t ggt_launch_integrate(const GgtIntegrateParams& p, int dtype, bool fused, cudaStream_t st);
+cudaError_t ggt_launch_extract(const GgtExtractParams& p, int dtype, cudaStream_t st);
+cudaError_t ggt_launch_export(const GgtExtractParams& p, int dtype, float* T, float* W, cudaStream_t st);

@@ -335,12 +335,21 @@ class Workload:
     # ---- per-frame inputs ------------------------------------------------------------------------
     def view_inputs(self, frame: int, view: int):
         """(depth float32 HxW, rgb uint8 HxWx3 or None) for rig camera `view` at `frame`."""
+        cache = self.__dict__.setdefault("_cache", {})
+        if (frame, view) in cache:
+            return cache[(frame, view)]
         time = frame / self.fps
         d, rgb = raycast(self.rig[view], self.scene, time, want_colour=self.colour)
         st = stream_id(frame, view, 1)
         d = noisy_depth(d, self.seed, st, self.sigma, self.p_invalid)
         if rgb is not None:
             rgb = noisy_colour(rgb, self.seed, st)
+        d.setflags(write=False)
+        if rgb is not None:
+            rgb.setflags(write=False)
+        if len(cache) >= 48:              # bounded memo: both pipelines of a test ask for the same inputs
+            cache.pop(next(iter(cache)))
+        cache[(frame, view)] = (d, rgb)
         return d, rgb
 
     def true_depth(self, cam: Camera, frame: int) -> np.ndarray:
