@@ -1,0 +1,397 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line for the geometry-guidance hot path on N B200s.
+
+A step = one pass of the whole hot path over one target frame of the workload (default: C3 =
+BASELINE.json:configs[2], 1920x1080 target, D = 128 inverse-depth bins, V = 4 input views of 1920x1080):
+ggt_refine_depth on each of the V views, ggt_integrate (weight maps + fusion), ggt_extract_depth.
+  value     Gvoxel.view/s = W_t*H_t*D*V per step / whole-step device time (inputs resident in HBM)
+  e2e       same metric through ggt_frame_host with pinned HOST buffers (H2D of colour + depth, D2H of
+            depth + confidence inside the timed region)
+  roofline  dominant kernel (integrate main) timed with CUDA events on its stream via ggt_profile_*
+  cpu_baseline  the oracle as it stands on the host cores, bounded sample
+`--impl reference` times the oracle (tier contract: the reference arm is the oracle).
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "Gvoxel·view TSDF updates/s"
+UNIT = "Gvoxel·view/s"
+REFINE = dict(lambda_t=0.7, beta=0.6, theta=8.0 / 255.0)
+N_INPUT_FRAMES = 3          # distinct synthetic frames cycled through (prev/cur pairs)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C3", choices=["C2", "C3", "C4"])
+    ap.add_argument("--fused", action="store_true", help="use ggt_integrate_extract instead of integrate + extract")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            d = json.load(fh)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", d
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)", {}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons during the timed region (pynvml, ~5 ms period)."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag, self.max_mhz = index, [], set(), False, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+                 0x80: "hw_power_brake", 0x2: "applications_clocks_setting"}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(0.005)
+
+    def result(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def physical_gpu_index(local_rank):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+# ----------------------------------------------------------------------------------------------------
+# workload set-up (inputs generated on the host by the seeded generator, then made resident in HBM)
+# ----------------------------------------------------------------------------------------------------
+class Inputs:
+    def __init__(self, name, rank, world):
+        from paper_2505_18932_b200 import sharding, synth
+        self.wl = wl = synth.workload(name)
+        self.frames = sharding.frames_for_rank(rank, world, N_INPUT_FRAMES)
+        self.target = wl.targets(self.frames[0])[0]
+        self.vi = wl.views_for(self.target)
+        self.views = [wl.rig[v] for v in self.vi]
+        self.data = [[wl.view_inputs(f, v) for v in self.vi] for f in self.frames]   # [frame][view] -> (depth, rgb)
+        self.W, self.H = self.views[0].width, self.views[0].height
+        self.V = len(self.vi)
+        self.vv_per_step = float(self.target.width) * self.target.height * wl.z_bins.size * self.V
+
+    def describe(self, world):
+        wl, t = self.wl, self.target
+        return {"workload": "%s (BASELINE.json:configs[%d]): target %dx%d, D=%d inverse-depth bins [0.5,5] m, V=%d views "
+                            "of %dx%d from the 16-camera grid rig, %s %s volume, refine=%s"
+                            % (wl.name, int(wl.name[1]) - 1, t.width, t.height, wl.z_bins.size, self.V, self.W, self.H,
+                               wl.storage, "persistent" if wl.persistent else "overwrite", wl.colour),
+                "targets_per_step": 1, "views": self.V, "bins": int(wl.z_bins.size),
+                "parallelism": "independent target streams per GPU x%d (no data-path collective)" % world,
+                "l2": "per-step traffic (volume %.2f GB written + read) exceeds the 126 MB L2; no explicit flush"
+                      % (t.width * t.height * wl.z_bins.size * (4 if wl.storage == "f16" else 8) / 1e9)}
+
+
+class DeviceRun:
+    """Device-resident inputs and the step function (all compute in libggt.so kernels)."""
+
+    def __init__(self, inp, fused):
+        import torch
+        from paper_2505_18932_b200 import binding
+        self.torch, self.b, self.inp, self.fused = torch, binding, inp, fused
+        wl = inp.wl
+        self.ctx = binding.Context()
+        self.ctx.ggt_set_workspace(inp.V, inp.W, inp.H)
+        self.vol = self.ctx.ggt_volume_bind(inp.target.width, inp.target.height, wl.z_bins,
+                                            dtype=binding.GGT_F16 if wl.storage == "f16" else binding.GGT_F32,
+                                            trunc_bins=wl.trunc_bins, weight_cap=wl.weight_cap)
+        self.vol.ggt_volume_reset()
+        self.depth_in = [[torch.from_numpy(np.array(d)).cuda() for d, _ in fr] for fr in inp.data]
+        self.rgb_in = [[torch.from_numpy(np.array(r)).cuda() if r is not None else None for _, r in fr] for fr in inp.data]
+        self.state = [self.depth_in[0][k].clone() for k in range(inp.V)]
+        n = inp.target.width * inp.target.height
+        self.depth = torch.empty(n, dtype=torch.float32, device="cuda")
+        self.conf = torch.empty(n, dtype=torch.float32, device="cuda")
+        self.flags = binding.GGT_ACCUMULATE if wl.persistent else binding.GGT_OVERWRITE
+        self.i = 0
+
+    def step(self):
+        inp, ctx = self.inp, self.ctx
+        cur = 1 + self.i % (N_INPUT_FRAMES - 1)
+        prev = cur - 1
+        self.i += 1
+        if inp.wl.colour:
+            for k in range(inp.V):
+                ctx.ggt_refine_depth(self.rgb_in[cur][k], self.rgb_in[prev][k], self.depth_in[cur][k], self.state[k], **REFINE)
+            depths = self.state
+        else:
+            depths = self.depth_in[cur]
+        if self.fused:
+            ctx.ggt_integrate_extract(self.vol, inp.target, inp.views, depths, self.flags, self.depth, self.conf)
+        else:
+            ctx.ggt_integrate(self.vol, inp.target, inp.views, depths, self.flags)
+            ctx.ggt_extract_depth(self.vol, self.depth, self.conf)
+
+
+class HostRun:
+    """End-to-end through ggt_frame_host: pinned host inputs/outputs, copies inside the timed region."""
+
+    def __init__(self, inp, dev: DeviceRun):
+        import ctypes
+        import torch
+        self.torch, self.inp, self.dev = torch, inp, dev
+        wl = inp.wl
+        self.rgb = [[torch.from_numpy(np.array(r)).pin_memory() if r is not None else None for _, r in fr] for fr in inp.data]
+        self.dep = [[torch.from_numpy(np.array(d)).pin_memory() for d, _ in fr] for fr in inp.data]
+        n = inp.target.width * inp.target.height
+        self.out_d = torch.empty(n, dtype=torch.float32).pin_memory()
+        self.out_c = torch.empty(n, dtype=torch.float32).pin_memory()
+        nb = dev.ctx.lib.ggt_frame_staging_bytes(ctypes.byref(dev.vol.desc), inp.V, inp.V, inp.W, inp.H)
+        self.staging = torch.empty(nb, dtype=torch.uint8, device="cuda")
+        self.slot_state = np.zeros(inp.V, np.uint32)
+        self.prm = dev.b.ggt_refine_params(REFINE["lambda_t"], REFINE["beta"], REFINE["theta"], 4, 3) if wl.colour else None
+        self.h2d = inp.V * (inp.W * inp.H * 4 + (inp.W * inp.H * 3 if wl.colour else 0))
+        self.d2h = 2 * n * 4
+        self.i = 0
+
+    def step(self):
+        inp, dev = self.inp, self.dev
+        cur = self.i % N_INPUT_FRAMES
+        self.i += 1
+        dev.ctx.ggt_frame_host(dev.vol, inp.target, inp.views, self.rgb[cur] if inp.wl.colour else None, self.dep[cur],
+                               list(range(inp.V)), self.slot_state, self.staging, self.out_d, self.out_c,
+                               flags=dev.flags, refine_params=self.prm)
+
+
+def timed(torch, dist, fn, steps, warmup):
+    """W untimed steps, then exactly K steps between barrier + synchronize, CUDA events on the current stream."""
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    return e0.elapsed_time(e1)
+
+
+# ----------------------------------------------------------------------------------------------------
+# the oracle, timed as it stands on the host cores (cpu_baseline leg and --impl reference)
+# ----------------------------------------------------------------------------------------------------
+def oracle_step(inp, ray_every, cur=1):
+    """One step of the whole path on the CPU oracle: refine + weight maps in full for the V views,
+    integrate + extract on a seeded 1/ray_every subset of the target rays.  Returns the wall time
+    extrapolated to the full frame (ray-dependent part scaled by the sampling ratio) and its parts."""
+    import oracle
+    wl, tgt = inp.wl, inp.target
+    t0 = time.perf_counter()
+    depths = []
+    for k in range(inp.V):
+        d, rgb = inp.data[cur][k]
+        if wl.colour:
+            dp, rp = inp.data[cur - 1][k]
+            d = oracle.refine(rgb, rp, d, dp, want_mask=False, **REFINE)[0]
+        depths.append(d)
+    t1 = time.perf_counter()
+    maps = [oracle.weight_map(d) for d in depths]
+    t2 = time.perf_counter()
+    n = tgt.width * tgt.height
+    rays = np.arange(ray_every // 2, n, ray_every, dtype=np.int32)
+    tau = oracle.tau_table(wl.z_bins, wl.trunc_bins)
+    T, W = oracle.integrate(tgt, wl.z_bins, tau, inp.views, maps, rays=rays, accumulate=wl.persistent,
+                            cap=wl.weight_cap, half_storage=wl.storage == "f16")
+    oracle.extract(wl.z_bins, T, W)
+    t3 = time.perf_counter()
+    scale = n / float(rays.size)
+    full = (t1 - t0) + (t2 - t1) + (t3 - t2) * scale
+    return full, {"refine_s": t1 - t0, "weight_s": t2 - t1, "integrate_extract_sample_s": t3 - t2,
+                  "rays": int(rays.size), "measured_s": t3 - t0}
+
+
+def cpu_baseline(inp, ray_every=8):
+    full, parts = oracle_step(inp, ray_every)
+    return {"value": inp.vv_per_step / full / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "one %s step: refine + weight maps of all %d views in full, integrate + extract on every %dth "
+                      "target ray (%d rays), ray part scaled by the sampling ratio; %.1f s of CPU work, "
+                      "extrapolated %.1f s per frame; host has %d cores, the oracle is single-threaded"
+                      % (inp.wl.name, inp.V, ray_every, parts["rays"], parts["measured_s"], full, os.cpu_count() or 0),
+            "ms_per_step_extrapolated": full * 1e3}
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle on the host cores (rank 0 only), same metric / config."""
+    if rank != 0:
+        return
+    inp = Inputs(args.workload, 0, 1)
+    ray_every = 64
+    for _ in range(min(args.warmup, 1)):
+        oracle_step(inp, ray_every)
+    fulls, parts = [], None
+    steps = max(1, min(args.steps, 5))           # bounded: each sampled step is ~6 s of CPU work
+    for i in range(steps):
+        full, parts = oracle_step(inp, ray_every, cur=1 + i % (N_INPUT_FRAMES - 1))
+        fulls.append(full)
+    ms = float(np.mean(fulls)) * 1e3
+    value = inp.vv_per_step / (ms / 1e3) / 1e9
+    sample = ("each step: refine + weight maps of all %d views in full, integrate + extract on every %dth ray (%d rays), "
+              "extrapolated to the frame; %d of the requested %d steps run (bounded)" % (inp.V, ray_every, parts["rays"], steps, args.steps))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": min(args.warmup, 1), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": inp.describe(1),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------------------------------
+def main():
+    args = parse_args()
+    from paper_2505_18932_b200 import sharding
+    rank, local_rank, world = sharding.env_rank()
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        torch.cuda.set_device(local_rank)
+        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist = dist_mod
+    else:
+        torch.cuda.set_device(0)
+    import __graft_entry__
+    if rank == 0:
+        __graft_entry__.build()
+    if dist is not None:
+        dist.barrier()
+
+    inp = Inputs(args.workload, rank, world)
+    dev = DeviceRun(inp, args.fused)
+    host = HostRun(inp, dev)
+    hbm_peak, peak_src, _ = measured_peaks()
+
+    # ---- headline: device-resident inputs --------------------------------------------------------------
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    launches0 = dev.ctx.launch_count
+    for _ in range(args.warmup):
+        dev.step()
+    launches_w = dev.ctx.launch_count
+    sampler.start()
+    ms_local = timed(torch, dist, dev.step, args.steps, 0)
+    sampler.stop_flag = True
+    sampler.join(timeout=2)
+    gpu_launches = dev.ctx.launch_count - launches_w
+    red = sharding.reduce_timing(ms_local, inp.vv_per_step * args.steps, device="cuda" if dist is not None else None)
+    ms_per_step = red["ms"] / args.steps
+    value = red["units"] / (red["ms"] / 1e3) / 1e9
+
+    # ---- per-stage device time of the same step (events around each kernel group, same stream) ---------
+    dev.ctx.ggt_profile_enable(True)
+    torch.cuda.synchronize()
+    for _ in range(args.steps):
+        dev.step()
+    torch.cuda.synchronize()
+    prof = dev.ctx.ggt_profile_collect()
+    dev.ctx.ggt_profile_enable(False)
+    stage_ms = {k: (v[0] / max(args.steps, 1)) for k, v in prof.items()}
+    t, wl = inp.target, inp.wl
+    voxels = t.width * t.height * wl.z_bins.size
+    vox_bytes = voxels * (4 if wl.storage == "f16" else 8)
+    map_bytes = inp.V * inp.W * inp.H * 8
+    integ_bytes = vox_bytes * (2 if wl.persistent else 1) + map_bytes      # algorithmic: DESIGN.md "Roofline"
+    integ_ms = prof["integrate"][0] / max(prof["integrate"][1], 1)
+    achieved = integ_bytes / (integ_ms / 1e3) / 1e9 if integ_ms > 0 else 0.0
+    path_bytes = integ_bytes + (0 if args.fused else vox_bytes) + 2 * t.width * t.height * 4
+    path_ms = stage_ms["integrate"] + stage_ms["extract"]
+    roofline = {"bound": "hbm", "kernel": "k_integrate (ggt_integrate main kernel)", "achieved": achieved, "peak": hbm_peak,
+                "unit": "GB/s", "frac": achieved / hbm_peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": integ_bytes, "ms_per_launch": integ_ms,
+                "integrate_plus_extract": {"bytes": path_bytes, "ms": path_ms,
+                                           "frac": (path_bytes / (path_ms / 1e3) / 1e9 / hbm_peak) if path_ms > 0 else 0.0},
+                "alu": {"flop_per_voxel_view": 16, "achieved_tflops": 16 * inp.vv_per_step / (integ_ms / 1e3) / 1e12 if integ_ms > 0 else 0.0,
+                        "peak_tflops_at_max_clock": 148 * 128 * 2 * 1.965e9 / 1e12}}
+    traffic_file = os.path.join(ROOT, "profiles", "traffic_integrate.json")
+    if os.path.exists(traffic_file):
+        with open(traffic_file) as fh:
+            roofline["traffic"] = json.load(fh).get(wl.name + ("_fused" if args.fused else ""))
+
+    # ---- e2e: host buffers through ggt_frame_host, result needed on the host every step ----------------
+    def e2e_step():
+        host.step()
+        torch.cuda.current_stream().synchronize()
+    e2e_steps = max(3, min(args.steps, 50))
+    ms_e2e_local = timed(torch, dist, e2e_step, e2e_steps, max(3, min(args.warmup, 5)))
+    red_e = sharding.reduce_timing(ms_e2e_local, inp.vv_per_step * e2e_steps, device="cuda" if dist is not None else None)
+    e2e = {"value": red_e["units"] / (red_e["ms"] / 1e3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": host.h2d,
+           "d2h_bytes_per_step": host.d2h, "ms_per_step": red_e["ms"] / e2e_steps, "steps": e2e_steps,
+           "api": "ggt_frame_host (pinned host buffers, stream synchronised every step)"}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32" if wl.storage == "f32" else "f32 compute, f16 storage", "data": "synthetic",
+                "config": inp.describe(world), "clocks": sampler.result(), "e2e": e2e, "gpu_launches": int(gpu_launches),
+                "roofline": roofline,
+                "stages_ms": {"refine_all_views": stage_ms["refine"], "weight_maps": stage_ms["weight"],
+                              "integrate": stage_ms["integrate"], "extract": stage_ms["extract"],
+                              "note": "per-step device time per stage (CUDA events on the launching stream)"},
+                "ms_per_1080p_target_frame": ms_per_step,
+                "integrate_gvoxel_view_per_s": inp.vv_per_step / (integ_ms / 1e3) / 1e9 if integ_ms > 0 else None,
+                "paper_context": "PAPER.md Table 4: TSDF stage 6 ms/frame at 1352x1014, K=4, GPU not stated"}
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = cpu_baseline(inp)
+        print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -90,6 +90,13 @@ const char* ggt_last_error(const ggt_ctx* ctx);
 /* Number of kernels this context has launched so far (bench.py's gpu_launches). */
 int64_t ggt_launch_count(const ggt_ctx* ctx);
 
+/* Optional per-stage device timing for bench.py's roofline: when enabled, every call records a pair of
+ * CUDA events on the caller's stream around its kernels.  ggt_profile_collect waits for them, writes the
+ * summed milliseconds and the number of timed groups per stage into host arrays of 4 entries
+ * (0 refine, 1 weight maps, 2 integrate main kernel, 3 extract) and clears the records. */
+int ggt_profile_enable(ggt_ctx* ctx, int32_t enable);
+int ggt_profile_collect(ggt_ctx* ctx, double* host_ms, int64_t* host_count);
+
 /* ---- workspace for the {depth, omega} maps of Eq. 11-12 ------------------------------------------ */
 /* Bytes of device scratch ggt_integrate needs for n_views maps of width x height: 8 B per pixel. */
 size_t ggt_workspace_bytes(int32_t n_views, int32_t width, int32_t height);

@@ -21,7 +21,7 @@ GGT_OVERWRITE, GGT_ACCUMULATE = 0, 1
 GGT_MAX_VIEWS = 16
 
 EXPORTS = [
-    "ggt_create", "ggt_destroy", "ggt_last_error", "ggt_launch_count", "ggt_workspace_bytes", "ggt_set_workspace",
+    "ggt_create", "ggt_destroy", "ggt_last_error", "ggt_launch_count", "ggt_profile_enable", "ggt_profile_collect", "ggt_workspace_bytes", "ggt_set_workspace",
     "ggt_volume_bytes", "ggt_volume_bind", "ggt_volume_unbind", "ggt_volume_reset", "ggt_volume_export",
     "ggt_volume_tables", "ggt_refine_depth", "ggt_integrate", "ggt_extract_depth", "ggt_integrate_extract",
     "ggt_frame_staging_bytes", "ggt_frame_host",
@@ -71,6 +71,8 @@ def load_library() -> ctypes.CDLL:
     lib.ggt_last_error.restype = ctypes.c_char_p
     lib.ggt_launch_count.argtypes = [vp]
     lib.ggt_launch_count.restype = ctypes.c_int64
+    lib.ggt_profile_enable.argtypes = [vp, i32]
+    lib.ggt_profile_collect.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64)]
     lib.ggt_workspace_bytes.argtypes = [i32, i32, i32]
     lib.ggt_workspace_bytes.restype = ctypes.c_size_t
     lib.ggt_set_workspace.argtypes = [vp, vp, ctypes.c_size_t]
@@ -150,6 +152,16 @@ class Context:
     @property
     def launch_count(self) -> int:
         return int(self.lib.ggt_launch_count(self.h))
+
+    def ggt_profile_enable(self, enable: bool):
+        self.check(self.lib.ggt_profile_enable(self.h, int(enable)), "ggt_profile_enable")
+
+    def ggt_profile_collect(self):
+        """{stage: (total ms, groups)} for refine / weight / integrate / extract since the last collect."""
+        ms = (ctypes.c_double * 4)()
+        n = (ctypes.c_int64 * 4)()
+        self.check(self.lib.ggt_profile_collect(self.h, ms, n), "ggt_profile_collect")
+        return {k: (ms[i], int(n[i])) for i, k in enumerate(("refine", "weight", "integrate", "extract"))}
 
     def ggt_set_workspace(self, n_views: int, width: int, height: int):
         import torch

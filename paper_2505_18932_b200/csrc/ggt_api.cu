@@ -29,6 +29,23 @@ int cuda_fail(ggt_ctx* ctx, cudaError_t e, const char* what) {
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// RAII pair of events around one kernel group when ggt_profile_enable is on (no-op otherwise).
+struct StageTimer {
+    ggt_ctx* c; cudaStream_t st; ggt_ctx::ProfRec* r = nullptr;
+    StageTimer(ggt_ctx* ctx, int stage, cudaStream_t s) : c(ctx), st(s) {
+        if (!c->prof) return;
+        if (c->prof_used == c->prof_pool.size()) {
+            ggt_ctx::ProfRec n; n.stage = stage;
+            if (cudaEventCreate(&n.a) != cudaSuccess || cudaEventCreate(&n.b) != cudaSuccess) return;
+            c->prof_pool.push_back(n);
+        }
+        r = &c->prof_pool[c->prof_used++];
+        r->stage = stage;
+        cudaEventRecord(r->a, st);
+    }
+    ~StageTimer() { if (r) cudaEventRecord(r->b, st); }
+};
+
 // Relative transform of PAPER.md:331 in double, rounded once to float:
 //   p_world = R_t^T (z K_t^{-1} (uc, vc, 1)^T - t_t);  (x, y, w) = K_k (R_k p_world + t_k)
 //   => (x, y, w) = z * Hm (uc, vc, 1)^T + e  with  Hm = K_k R_k R_t^T K_t^{-1},  e = K_k (t_k - R_k R_t^T t_t).
@@ -113,6 +130,7 @@ int ggt_destroy(ggt_ctx* ctx) {
     ggt_ctx* c = ctx;
     if (c->ws_owned && c->ws) cudaFree(c->ws);
     if (c->cq) cudaFree(c->cq);
+    for (auto& r : c->prof_pool) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     delete c;
     return GGT_OK;
 }
@@ -120,6 +138,29 @@ int ggt_destroy(ggt_ctx* ctx) {
 const char* ggt_last_error(const ggt_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
 
 int64_t ggt_launch_count(const ggt_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int ggt_profile_enable(ggt_ctx* ctx, int32_t enable) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    ctx->prof = enable != 0;
+    ctx->prof_used = 0;
+    return GGT_OK;
+}
+
+int ggt_profile_collect(ggt_ctx* ctx, double* host_ms, int64_t* host_count) {
+    if (!ctx || !host_ms || !host_count) return GGT_ERR_INVALID_ARG;
+    for (int i = 0; i < GGT_N_STAGES; ++i) { host_ms[i] = 0.0; host_count[i] = 0; }
+    for (size_t i = 0; i < ctx->prof_used; ++i) {
+        ggt_ctx::ProfRec& r = ctx->prof_pool[i];
+        cudaError_t e = cudaEventSynchronize(r.b);
+        float ms = 0.0f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, r.a, r.b);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "ggt_profile_collect");
+        host_ms[r.stage] += ms;
+        host_count[r.stage] += 1;
+    }
+    ctx->prof_used = 0;
+    return GGT_OK;
+}
 
 size_t ggt_workspace_bytes(int32_t n_views, int32_t width, int32_t height) {
     if (n_views <= 0 || width <= 0 || height <= 0) return 0;
@@ -246,6 +287,7 @@ int ggt_refine_depth(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t*
         }
     }
     int n = 0;
+    StageTimer tm(ctx, GGT_STAGE_REFINE, (cudaStream_t)stream);
     cudaError_t e = ggt_launch_refine(width, height, dev_rgb_cur, dev_rgb_prev, rgb_pixel_stride, dev_depth_cur,
                                       dev_depth_state, dev_mask_out, dev_pooled_out, c->cq, params->lambda_t,
                                       params->beta, params->theta, (cudaStream_t)stream, &n);
@@ -291,6 +333,8 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
     p.tables = vol->dev_tables; p.voxels = vol->dev_voxels;
     p.depth = dev_depth; p.conf = dev_conf; p.bin = dev_bin;
     char* w = static_cast<char*>(ctx->ws);
+    {
+    StageTimer tm(ctx, GGT_STAGE_WEIGHT, st);
     for (int k = 0; k < n_views; ++k) {
         relative_transform(*target, views[k], p.v[k].h, p.v[k].e);
         p.v[k].map = reinterpret_cast<const float2*>(w);
@@ -301,6 +345,8 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
         ctx->launches += 1;
         w += align_up((size_t)views[k].width * views[k].height * sizeof(float2), 256);
     }
+    }
+    StageTimer tm(ctx, GGT_STAGE_INTEGRATE, st);
     cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, fused, st);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "integrate launch");
     ctx->launches += 1;
@@ -324,6 +370,7 @@ int ggt_extract_depth(ggt_ctx* ctx, const ggt_volume* vol, float* dev_depth, flo
     if (!vol) return fail(ctx, GGT_ERR_INVALID_ARG, "volume is NULL");
     GgtExtractParams p = extract_params(vol);
     p.depth = dev_depth; p.conf = dev_conf; p.bin = dev_bin;
+    StageTimer tm(ctx, GGT_STAGE_EXTRACT, (cudaStream_t)stream);
     cudaError_t e = ggt_launch_extract(p, vol->desc.dtype, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "extract launch");
     ctx->launches += 1;

@@ -50,7 +50,14 @@ struct ggt_ctx {
     bool ws_owned = false;
     uint16_t* cq = nullptr;        // quarter-res block differences of ggt_refine_depth (context-owned)
     size_t cq_bytes = 0;
+    // optional per-stage device timing (ggt_profile_enable): pairs of events around each kernel group
+    bool prof = false;
+    struct ProfRec { int stage; cudaEvent_t a, b; };
+    std::vector<ProfRec> prof_pool;
+    size_t prof_used = 0;
 };
+
+enum { GGT_STAGE_REFINE = 0, GGT_STAGE_WEIGHT = 1, GGT_STAGE_INTEGRATE = 2, GGT_STAGE_EXTRACT = 3, GGT_N_STAGES = 4 };
 
 struct ggt_volume {
     ggt_volume_desc desc;

@@ -103,12 +103,12 @@ def test_C4_full_size_sampled():
 
 
 def test_C5_scaled_batched_targets_all_rays():
-    run_config("C5", 0.125, [0, 1, 2], 1)
+    run_config("C5", 0.125, [0, 1, 2], 1, expect_hits=0.2)   # 90-degree targets see beyond the rig's coverage
 
 
 def test_C5_full_size_sampled():
     # 8 persistent fp32 volumes of 2048 x 2048 x 128 (34.4 GB), 1/512 of the rays, 2 frames
-    run_config("C5", 1.0, [0, 1], 512)
+    run_config("C5", 1.0, [0, 1], 512, expect_hits=0.2)
 
 
 def test_fused_persistent_fp16_matches():
