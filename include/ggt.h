@@ -97,8 +97,16 @@ int64_t ggt_launch_count(const ggt_ctx* ctx);
 int ggt_profile_enable(ggt_ctx* ctx, int32_t enable);
 int ggt_profile_collect(ggt_ctx* ctx, double* host_ms, int64_t* host_count);
 
+/* Test hook (determinism contract, P14): the integrate kernel forms 1/w and A/W with its own
+ * branch-free packed sequences; this runs them on n pairs (dev_a[i], dev_b[i]), b > 0, and ADDS to
+ * dev_mismatch[0] / [1] the number of elements whose reciprocal 1/b / quotient a/b differ in any bit from the
+ * IEEE-754 round-to-nearest results (__frcp_rn, __fdiv_rn).  n even; dev_mismatch zeroed by the caller. */
+int ggt_selftest_arith(ggt_ctx* ctx, int64_t n, const float* dev_a, const float* dev_b, uint32_t* dev_mismatch,
+                       void* stream);
+
 /* ---- workspace for the {depth, omega} maps of Eq. 11-12 ------------------------------------------ */
-/* Bytes of device scratch ggt_integrate needs for n_views maps of width x height: 8 B per pixel. */
+/* Bytes of device scratch ggt_integrate needs for n_views maps of width x height: 8 B per record of the
+ * zero-padded (height+1) x (width+1) {depth, omega} map, each map rounded up to 256 B. */
 size_t ggt_workspace_bytes(int32_t n_views, int32_t width, int32_t height);
 /* Hands caller-owned device scratch to the context.  Without it (or if it is too small) ggt_integrate
  * grows an internal cudaMalloc'ed buffer, which synchronises the device once per growth. */

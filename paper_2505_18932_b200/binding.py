@@ -21,7 +21,7 @@ GGT_OVERWRITE, GGT_ACCUMULATE = 0, 1
 GGT_MAX_VIEWS = 16
 
 EXPORTS = [
-    "ggt_create", "ggt_destroy", "ggt_last_error", "ggt_launch_count", "ggt_profile_enable", "ggt_profile_collect", "ggt_workspace_bytes", "ggt_set_workspace",
+    "ggt_create", "ggt_destroy", "ggt_last_error", "ggt_launch_count", "ggt_profile_enable", "ggt_profile_collect", "ggt_selftest_arith", "ggt_workspace_bytes", "ggt_set_workspace",
     "ggt_volume_bytes", "ggt_volume_bind", "ggt_volume_unbind", "ggt_volume_reset", "ggt_volume_export",
     "ggt_volume_tables", "ggt_refine_depth", "ggt_integrate", "ggt_extract_depth", "ggt_integrate_extract",
     "ggt_frame_staging_bytes", "ggt_frame_host",
@@ -73,6 +73,7 @@ def load_library() -> ctypes.CDLL:
     lib.ggt_launch_count.restype = ctypes.c_int64
     lib.ggt_profile_enable.argtypes = [vp, i32]
     lib.ggt_profile_collect.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64)]
+    lib.ggt_selftest_arith.argtypes = [vp, ctypes.c_int64, vp, vp, vp, vp]
     lib.ggt_workspace_bytes.argtypes = [i32, i32, i32]
     lib.ggt_workspace_bytes.restype = ctypes.c_size_t
     lib.ggt_set_workspace.argtypes = [vp, vp, ctypes.c_size_t]
@@ -162,6 +163,15 @@ class Context:
         n = (ctypes.c_int64 * 4)()
         self.check(self.lib.ggt_profile_collect(self.h, ms, n), "ggt_profile_collect")
         return {k: (ms[i], int(n[i])) for i, k in enumerate(("refine", "weight", "integrate", "extract"))}
+
+    def ggt_selftest_arith(self, a, b):
+        """(reciprocal mismatches, division mismatches) of the kernel's arithmetic vs IEEE on cuda tensors a, b."""
+        import torch
+        out = torch.zeros(2, dtype=torch.int32, device="cuda")
+        self.check(self.lib.ggt_selftest_arith(self.h, a.numel(), a.data_ptr(), b.data_ptr(), out.data_ptr(), _stream()),
+                   "ggt_selftest_arith")
+        r = out.cpu().numpy()
+        return int(r[0]), int(r[1])
 
     def ggt_set_workspace(self, n_views: int, width: int, height: int):
         import torch

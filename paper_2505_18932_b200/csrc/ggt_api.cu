@@ -162,9 +162,17 @@ int ggt_profile_collect(ggt_ctx* ctx, double* host_ms, int64_t* host_count) {
     return GGT_OK;
 }
 
+int ggt_selftest_arith(ggt_ctx* ctx, int64_t n, const float* dev_a, const float* dev_b, uint32_t* dev_mismatch, void* stream) {
+    if (!ctx || !dev_a || !dev_b || !dev_mismatch || n < 0) return GGT_ERR_INVALID_ARG;
+    cudaError_t e = ggt_launch_selftest_arith(n, dev_a, dev_b, dev_mismatch, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "ggt_selftest_arith");
+    ctx->launches += 1;
+    return GGT_OK;
+}
+
 size_t ggt_workspace_bytes(int32_t n_views, int32_t width, int32_t height) {
     if (n_views <= 0 || width <= 0 || height <= 0) return 0;
-    return (size_t)n_views * align_up((size_t)width * height * sizeof(float2), 256);
+    return (size_t)n_views * align_up(((size_t)width + 1) * ((size_t)height + 1) * sizeof(float2), 256);
 }
 
 int ggt_set_workspace(ggt_ctx* ctx, void* dev_workspace, size_t bytes) {
@@ -310,10 +318,10 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
     if (!(target->fx > 0.0f) || !(target->fy > 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "target focal length");
     size_t need = 0;
     for (int k = 0; k < n_views; ++k) {
-        if (views[k].width <= 0 || views[k].height <= 0 || views[k].width > (1 << 20) || views[k].height > (1 << 20))
+        if (views[k].width <= 0 || views[k].height <= 0 || views[k].width > 32767 || views[k].height > 32767)
             return fail(ctx, GGT_ERR_SHAPE, "view %d size %dx%d", k, views[k].width, views[k].height);
         if (!dev_depths[k]) return fail(ctx, GGT_ERR_INVALID_ARG, "dev_depths[%d] is NULL", k);
-        need += align_up((size_t)views[k].width * views[k].height * sizeof(float2), 256);
+        need += align_up(((size_t)views[k].width + 1) * ((size_t)views[k].height + 1) * sizeof(float2), 256);
     }
     if (ctx->ws_bytes < need) {
         if (ctx->ws && !ctx->ws_owned) return fail(ctx, GGT_ERR_SHAPE, "workspace %zu B < required %zu B", ctx->ws_bytes, need);
@@ -336,14 +344,19 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
     {
     StageTimer tm(ctx, GGT_STAGE_WEIGHT, st);
     for (int k = 0; k < n_views; ++k) {
-        relative_transform(*target, views[k], p.v[k].h, p.v[k].e);
+        float hm[9], ev[3];
+        relative_transform(*target, views[k], hm, ev);
+        for (int i = 0; i < 6; ++i) p.v[k].nh[i] = -hm[i];
+        for (int i = 0; i < 3; ++i) p.v[k].h2[i] = hm[6 + i];
+        p.v[k].ne[0] = -ev[0]; p.v[k].ne[1] = -ev[1]; p.v[k].e2 = ev[2];
         p.v[k].map = reinterpret_cast<const float2*>(w);
         p.v[k].width = views[k].width; p.v[k].height = views[k].height;
+        p.v[k].stride = (uint32_t)views[k].width + 1u;
         cudaError_t e = ggt_launch_weight_map(views[k].width, views[k].height, dev_depths[k], reinterpret_cast<float2*>(w),
                                               vol->desc.w_sigma0, vol->desc.w_clip, vol->desc.w_window, st);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "weight-map launch");
         ctx->launches += 1;
-        w += align_up((size_t)views[k].width * views[k].height * sizeof(float2), 256);
+        w += align_up(((size_t)views[k].width + 1) * ((size_t)views[k].height + 1) * sizeof(float2), 256);
     }
     }
     StageTimer tm(ctx, GGT_STAGE_INTEGRATE, st);

@@ -9,11 +9,15 @@
 #include "../../include/ggt.h"
 
 // ---- device-side parameter blocks (passed by value as __grid_constant__ kernel parameters) --------
-struct GgtViewParams {
-    float h[9];            // H_k = K_k R_k R_t^T K_t^{-1}   (row-major)
-    float e[3];            // e_k = K_k (t_k - R_k R_t^T t_t)
-    const float2* map;     // interleaved {depth, omega}, height x width
+struct GgtViewParams {      // (x, y, w) = z * H_k (uc, vc, 1)^T + e_k,  H_k = K_k R_k R_t^T K_t^{-1},  e_k = K_k (t_k - R_k R_t^T t_t)
+    float nh[6];           // rows 0-1 of H_k, NEGATED (the kernel carries -x, -y and -1/w: see ggt_integrate.cu)
+    float h2[3];           // row 2 of H_k
+    float ne[2];           // -e_k[0], -e_k[1]
+    float e2;              // e_k[2]
+    const float2* map;     // interleaved {depth (0 if invalid), omega (0 if invalid)}, height x width
     int32_t width, height;
+    uint32_t stride;       // records per map row = width + 1 (zero padding column)
+    int32_t pad_;
 };
 
 struct GgtIntegrateParams {
@@ -82,3 +86,4 @@ cudaError_t ggt_launch_weight_map(int W, int H, const float* depth, float2* out,
 cudaError_t ggt_launch_integrate(const GgtIntegrateParams& p, int dtype, bool fused, cudaStream_t st);
 cudaError_t ggt_launch_extract(const GgtExtractParams& p, int dtype, cudaStream_t st);
 cudaError_t ggt_launch_export(const GgtExtractParams& p, int dtype, float* T, float* W, cudaStream_t st);
+cudaError_t ggt_launch_selftest_arith(long long n, const float* a, const float* b, unsigned* mismatch, cudaStream_t st);

@@ -4,7 +4,8 @@
 // and packing of {depth, omega} into one 8-byte record per pixel so that the integrate kernel needs a single
 // gather per voxel.view.  Reading P11: missing / invalid neighbours contribute clip^2; nu == 0 -> omega = 1.
 // The 49 terms are added in row-major window order in fp32 (the order the oracle states), so the result is
-// bit-reproducible.  One CTA = 32 x 8 pixels, depth tile + 3-pixel halo staged in shared memory.
+// bit-reproducible.  The output is padded to (H+1) x (W+1) records, the extra column and row holding {0, 0}.
+// One CTA = 32 x 8 pixels, depth tile + 3-pixel halo staged in shared memory.
 #include "ggt_internal.h"
 
 namespace {
@@ -27,7 +28,12 @@ k_weight_map(int W, int H, const float* __restrict__ depth, float2* __restrict__
     }
     __syncthreads();
     const int x = x0 + tx, y = y0 + ty;
-    if (x >= W || y >= H) return;
+    if (x > W || y > H) return;
+    const size_t Ws = (size_t)W + 1;                      // padded record stride (see ggt_integrate.cu view_pair)
+    if (x == W || y == H) {                               // zero column / row the clamped gathers land on
+        out[(size_t)y * Ws + x] = make_float2(0.0f, 0.0f);
+        return;
+    }
     const float D0 = s_d[ty + R][tx + R];
     float omega;
     if (!(D0 > 0.0f)) {
@@ -56,14 +62,14 @@ k_weight_map(int W, int H, const float* __restrict__ depth, float2* __restrict__
             omega = w < 1.0f ? w : 1.0f;
         }
     }
-    out[(size_t)y * W + x] = make_float2(D0, omega);
+    out[(size_t)y * Ws + x] = make_float2(D0 > 0.0f ? D0 : 0.0f, omega);   // invalid -> {0, 0}: zero weight, finite depth
 }
 
 }  // namespace
 
 cudaError_t ggt_launch_weight_map(int W, int H, const float* depth, float2* out, float sigma0, float clip,
                                   int window, cudaStream_t st) {
-    const dim3 blk(BW, BH), grd((W + BW - 1) / BW, (H + BH - 1) / BH);
+    const dim3 blk(BW, BH), grd((W + 1 + BW - 1) / BW, (H + 1 + BH - 1) / BH);   // + the padding column / row
     const float c2 = clip * clip;   // one fp32 multiply, as the oracle states it
     k_weight_map<<<grd, blk, 0, st>>>(W, H, depth, out, sigma0, c2, window);
     return cudaGetLastError();

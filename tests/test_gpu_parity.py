@@ -31,6 +31,32 @@ def run_config(name, scale, frames, every, fused=False, expect_hits=0.5):
     return all_stats
 
 
+# ---- the kernel's own reciprocal / division against IEEE (determinism contract P14) -----------------------
+def test_fast_reciprocal_and_division():
+    import torch
+    from paper_2505_18932_b200 import binding
+    ctx = binding.Context()
+    # every float from 1e-6 (the validity threshold on w) up to 2^24, in chunks
+    lo = int(np.float32(1e-6).view(np.uint32)) & ~1
+    hi = int(np.float32(16777216.0).view(np.uint32))
+    g = torch.Generator(device="cuda").manual_seed(7)
+    total = 0
+    for start in range(lo, hi, 1 << 26):
+        bits = torch.arange(start, min(start + (1 << 26), hi), dtype=torch.int32, device="cuda")
+        b = bits.view(torch.float32)
+        # numerators: |a| <= 16 * b-ish magnitudes as in a weighted mean, random sign, plus exact zeros
+        a = (torch.rand(b.shape, generator=g, device="cuda") * 2 - 1) * b * 0.3
+        a[::97] = 0.0
+        r, q = ctx.ggt_selftest_arith(a, b)
+        assert r == 0 and q == 0, (start, r, q)
+        total += b.numel()
+    assert total > 3e8
+    # weights and numerators in the ranges the TSDF tail sees: Wn in [0.05, 16], |A| <= tau * Wn
+    b = torch.rand(1 << 24, generator=g, device="cuda") * 16 + 0.05
+    a = (torch.rand(1 << 24, generator=g, device="cuda") * 2 - 1) * b * 0.25
+    assert ctx.ggt_selftest_arith(a, b) == (0, 0)
+
+
 # ---- refine (a1-a2) ---------------------------------------------------------------------------------
 @pytest.mark.parametrize("W,H,stride", [(64, 48, 3), (200, 136, 3), (203, 131, 3), (132, 70, 4), (1920, 1080, 3)])
 def test_refine_parity(W, H, stride):
