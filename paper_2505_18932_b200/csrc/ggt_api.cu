@@ -360,6 +360,9 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
     }
     }
     StageTimer tm(ctx, GGT_STAGE_INTEGRATE, st);
+    p.same_size = 1;
+    for (int k = 1; k < n_views; ++k)
+        if (views[k].width != views[0].width || views[k].height != views[0].height) p.same_size = 0;
     cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, fused, st);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "integrate launch");
     ctx->launches += 1;

@@ -25,6 +25,8 @@ struct GgtIntegrateParams {
     int32_t n_views;
     int32_t n_groups;      // ceil(D / G)
     int32_t accumulate;    // 0 overwrite, 1 running average
+    int32_t same_size;     // 1 if all views have the same width x height
+    int32_t pad_;
     float decay, cap;
     const float* tables;   // device: z[0..Dpad) then tau[0..Dpad), Dpad = n_groups * G
     void* voxels;          // device: [n_groups][Ht][Wt][G][{T,W}]
