@@ -336,6 +336,7 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
     memset(&p, 0, sizeof p);
     p.Wt = vol->desc.width; p.Ht = vol->desc.height; p.D = vol->desc.bins;
     p.n_views = n_views; p.n_groups = vol->n_groups;
+    p.plane = (unsigned long long)vol->desc.width * (unsigned long long)vol->desc.height;
     p.accumulate = flags == GGT_ACCUMULATE ? 1 : 0;
     p.decay = vol->desc.decay; p.cap = vol->desc.weight_cap;
     p.tables = vol->dev_tables; p.voxels = vol->dev_voxels;
@@ -363,6 +364,10 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
     p.same_size = 1;
     for (int k = 1; k < n_views; ++k)
         if (views[k].width != views[0].width || views[k].height != views[0].height) p.same_size = 0;
+    // parallel rig: w_k(z) = fma(z, fma(h20, uc, fma(h21, vc, h22)), e2) has the same bits in every view
+    p.shared_w = p.same_size && n_views >= 2;
+    for (int k = 1; k < n_views; ++k)
+        if (memcmp(p.v[k].h2, p.v[0].h2, sizeof p.v[0].h2) != 0 || memcmp(&p.v[k].e2, &p.v[0].e2, sizeof(float)) != 0) p.shared_w = 0;
     cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, fused, st);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "integrate launch");
     ctx->launches += 1;
