@@ -344,6 +344,10 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
     char* w = static_cast<char*>(ctx->ws);
     {
     StageTimer tm(ctx, GGT_STAGE_WEIGHT, st);
+    GgtWeightParams wp;
+    memset(&wp, 0, sizeof wp);
+    wp.n_views = n_views; wp.window = vol->desc.w_window;
+    wp.sigma0 = vol->desc.w_sigma0; wp.c2 = vol->desc.w_clip * vol->desc.w_clip;
     for (int k = 0; k < n_views; ++k) {
         float hm[9], ev[3];
         relative_transform(*target, views[k], hm, ev);
@@ -353,12 +357,13 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
         p.v[k].map = reinterpret_cast<const float2*>(w);
         p.v[k].width = views[k].width; p.v[k].height = views[k].height;
         p.v[k].stride = (uint32_t)views[k].width + 1u;
-        cudaError_t e = ggt_launch_weight_map(views[k].width, views[k].height, dev_depths[k], reinterpret_cast<float2*>(w),
-                                              vol->desc.w_sigma0, vol->desc.w_clip, vol->desc.w_window, st);
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "weight-map launch");
-        ctx->launches += 1;
+        wp.v[k].depth = dev_depths[k]; wp.v[k].out = reinterpret_cast<float2*>(w);
+        wp.v[k].width = views[k].width; wp.v[k].height = views[k].height;
         w += align_up(((size_t)views[k].width + 1) * ((size_t)views[k].height + 1) * sizeof(float2), 256);
     }
+    cudaError_t e = ggt_launch_weight_maps(wp, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "weight-map launch");
+    ctx->launches += 1;
     }
     StageTimer tm(ctx, GGT_STAGE_INTEGRATE, st);
     p.same_size = 1;

@@ -37,6 +37,18 @@ struct GgtIntegrateParams {
     GgtViewParams v[GGT_MAX_VIEWS];
 };
 
+struct GgtWeightView {
+    const float* depth;    // fp32 height x width, <= 0 (or NaN) = invalid
+    float2* out;           // (height + 1) x (width + 1) records {depth, omega}
+    int32_t width, height;
+};
+
+struct GgtWeightParams {    // all views of one ggt_integrate call: one launch, blockIdx.z = view
+    int32_t n_views, window;
+    float sigma0, c2;      // c2 = clip * clip (one fp32 multiply, as the oracle states it)
+    GgtWeightView v[GGT_MAX_VIEWS];
+};
+
 struct GgtExtractParams {
     int32_t Wt, Ht, D, n_groups;
     const float* tables;
@@ -84,8 +96,7 @@ cudaError_t ggt_launch_refine(int W, int H, const uint8_t* rgb_cur, const uint8_
                               const float* depth_cur, float* depth_state, float* mask_out,
                               uint16_t* pooled_out, uint16_t* cq_scratch, float lambda_t, float beta,
                               float theta, cudaStream_t st, int* n_launches);
-cudaError_t ggt_launch_weight_map(int W, int H, const float* depth, float2* out, float sigma0, float clip,
-                                  int window, cudaStream_t st);
+cudaError_t ggt_launch_weight_maps(const GgtWeightParams& p, cudaStream_t st);
 cudaError_t ggt_launch_integrate(const GgtIntegrateParams& p, int dtype, bool fused, cudaStream_t st);
 cudaError_t ggt_launch_extract(const GgtExtractParams& p, int dtype, cudaStream_t st);
 cudaError_t ggt_launch_export(const GgtExtractParams& p, int dtype, float* T, float* W, cudaStream_t st);
