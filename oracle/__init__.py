@@ -171,3 +171,28 @@ def extract(z_bins, T, Wt):
                     _p(Wt, ctypes.c_float), _p(depth, ctypes.c_float), _p(conf, ctypes.c_float),
                     _p(bins, ctypes.c_int32))
     return depth, conf, bins
+
+
+def raymarch(target, views: Sequence, maps: Sequence[np.ndarray], z_near, z_far, tau=0.02, step_scale=0.8,
+             min_step=1e-3, max_evals=4096, n_bisect=3, rays: Optional[np.ndarray] = None):
+    """O-M (the paper's own schedule). Returns (depth, conf, steps) per ray."""
+    lib = _load()
+    n_rays = int(target.width) * int(target.height) if rays is None else int(rays.size)
+    if rays is not None:
+        rays = np.ascontiguousarray(rays, dtype=np.int32)
+    V = len(views)
+    cams = (OrcCamera * max(V, 1))(*[_cam(c) for c in views])
+    maps = [np.ascontiguousarray(m, dtype=np.float32) for m in maps]
+    ptrs = (ctypes.POINTER(ctypes.c_float) * max(V, 1))(*[_p(m, ctypes.c_float) for m in maps])
+    depth = np.empty(n_rays, dtype=np.float32)
+    conf = np.empty(n_rays, dtype=np.float32)
+    steps = np.empty(n_rays, dtype=np.int32)
+    t = _cam(target)
+    rc = lib.orc_raymarch(ctypes.byref(t), ctypes.c_int32(V), cams, ptrs, ctypes.c_int64(n_rays),
+                          _p(rays, ctypes.c_int32), ctypes.c_float(z_near), ctypes.c_float(z_far),
+                          ctypes.c_float(tau), ctypes.c_float(step_scale), ctypes.c_float(min_step),
+                          ctypes.c_int32(max_evals), ctypes.c_int32(n_bisect), _p(depth, ctypes.c_float),
+                          _p(conf, ctypes.c_float), _p(steps, ctypes.c_int32))
+    if rc != 0:
+        raise ValueError("orc_raymarch rc=%d" % rc)
+    return depth, conf, steps

@@ -22,11 +22,15 @@
 //   339-341 Eq. 10 truncated weighted fusion                                -> orc_integrate
 //   343-348 Eq. 11-12 depth-variance weight, w = 7                          -> orc_weight_map
 //   348    omega_k = 0 if s_k < -tau; surface = change of sign of s         -> orc_integrate / orc_extract
+//   75, 348 the paper's own schedule: on-the-fly TSDF, advance 0.8 s, sign change,
+//          three bisection steps (no volume)                                 -> orc_raymarch
 //   356-360 Eq. 13-14 accumulated temporal weight with cap (analogue: P9)   -> orc_integrate (accumulate)
 //
 // Pins (tests/test_oracle_pins.py, -m "not gpu"): T1 analytic planes/spheres, T2 coincident camera,
 // T3 view-order invariance, T4 brute-force fp64 per-voxel, T5 Eq. 1 closed forms, T6 Eq. 2 EMA,
-// T7 Eq. 11-12 closed forms (0.050518), T8 cut/clamp sweep, T9 running-average closed form, T10 extract.
+// T7 Eq. 11-12 closed forms (0.050518), T8 cut/clamp sweep, T9 running-average closed form, T10 extract,
+// T11-T14 raymarch (planes / sphere closed form, dense fp64 first-crossing brute force, coincident camera,
+// closed-form evaluation counts).
 // Parity unpinned (choices, not derivable): the VALUES of tau in C2-C5 (P3), the
 // dead-zone threshold semantics (P6), decay/cap without mask gate (P9-P10), the border rule of
 // Eq. 12 (P11), the confidence output (P13).
@@ -412,3 +416,130 @@ int orc_extract(int64_t n_rays, int32_t D, const float* z, const float* T, const
 }
 
 }  // extern "C"
+
+// --------------------------------------------------------------------------------------------------
+// O-M  The paper's own schedule: image-based TSDF evaluated on the fly along each
+// target ray, no volume ("integrates depth along each ray on the fly and, thus, avoids creating
+// an explicit 3D voxel grid"; "We advance along the ray with a step size of 0.8s until a surface
+// intersection is detected. This is indicated by a change of sign in the value of s. We subsequently perform
+// three steps of a bisection search to refine the intersection depth.").
+//
+// s(z) at target depth z: the per-sample arithmetic of O-I steps 1-4 with tau_j = tau (PAPER.md:341,
+// tau = 0.02 m), normalised as in reading P2: s = sum(omega_k c_k) / sum(omega_k); "unobserved" if the sum of
+// weights is 0.  Readings for what the paper leaves open (M1-M6):
+//   M1 start at z = z_near, a ray is a miss once z > z_far or after max_evals evaluations of s;
+//   M2 advance by max(step_scale * s, min_step) after a positive sample (step_scale = 0.8; min_step > 0
+//      guarantees progress, since 0.8 s alone converges to the surface without ever crossing it);
+//   M3 an unobserved sample advances like free space, by max(step_scale * tau, min_step);
+//   M4 a crossing is a sample with s <= 0 whose PREVIOUS sample was observed and positive (no crossing
+//      across an unobserved sample, as P13); a non-positive sample without such a predecessor advances by
+//      min_step;
+//   M5 bisection: n_bisect times m = 0.5 (a + b); s(m) > 0 -> a = m; s(m) <= 0 -> b = m; an unobserved
+//      midpoint ends the refinement; depth = 0.5 (a + b);
+//   M6 confidence = sum of weights at the last non-positive sample b; steps = evaluations of s.
+// outputs per ray: depth (0 = miss), conf (0 = miss), steps.
+// --------------------------------------------------------------------------------------------------
+namespace {
+struct OrcRayEval {
+    int n_views;
+    const OrcCamera* views;
+    const float* const* maps;
+    const float (*b)[3];
+    const float (*ev)[3];
+    float tau;
+};
+
+// one evaluation of Eq. 9-10 at target depth z: returns A = sum(omega c), Wn = sum(omega)
+inline void orc_eval_s(const OrcRayEval& E, float z, float* A_out, float* W_out) {
+    float A = 0.0f, Wn = 0.0f;
+    for (int k = 0; k < E.n_views; ++k) {
+        const float x = fmaf(z, E.b[k][0], E.ev[k][0]);
+        const float y = fmaf(z, E.b[k][1], E.ev[k][1]);
+        const float w = fmaf(z, E.b[k][2], E.ev[k][2]);          // z_k of Eq. 9
+        if (w < 1e-6f) continue;
+        const float rcp = 1.0f / w;
+        const float px = x * rcp, py = y * rcp;
+        const float fxp = std::floor(px), fyp = std::floor(py);
+        if (!(fxp >= 0.0f) || !(fyp >= 0.0f) || !(fxp < (float)E.views[k].width) ||
+            !(fyp < (float)E.views[k].height)) continue;
+        const int ix = (int)fxp, iy = (int)fyp;
+        const float* m = E.maps[k] + 2 * ((int64_t)iy * E.views[k].width + ix);
+        const float Dk = m[0], om = m[1];
+        if (!(Dk > 0.0f)) continue;
+        const float s = Dk - w;                                  // reading P1
+        if (s < -E.tau) continue;                                // omega_k = 0 if s_k < -tau
+        const float c = s < E.tau ? s : E.tau;                   // clamp(s_k, -tau, tau)
+        A = fmaf(om, c, A);
+        Wn = Wn + om;
+    }
+    *A_out = A;
+    *W_out = Wn;
+}
+}  // namespace
+
+extern "C" int orc_raymarch(const OrcCamera* tgt, int32_t n_views, const OrcCamera* views,
+                            const float* const* maps, int64_t n_rays, const int32_t* rays, float z_near,
+                            float z_far, float tau, float step_scale, float min_step, int32_t max_evals,
+                            int32_t n_bisect, float* depth, float* conf, int32_t* steps) {
+    if (n_views < 0 || !(z_far > z_near) || !(tau > 0.0f) || !(min_step > 0.0f) || max_evals < 1 || n_bisect < 0)
+        return -1;
+    const int32_t Wd = tgt->width, Hd = tgt->height;
+    if (!rays) n_rays = (int64_t)Wd * Hd;
+    const int nv = n_views > 0 ? n_views : 1;
+    float (*Hm)[9] = new float[nv][9];
+    float (*ev)[3] = new float[nv][3];
+    float (*b)[3] = new float[nv][3];
+    for (int k = 0; k < n_views; ++k) orc_relative(tgt, &views[k], Hm[k], ev[k]);
+    const float free_step = fmaxf(step_scale * tau, min_step);   // M3
+    for (int64_t r = 0; r < n_rays; ++r) {
+        const int32_t pix = rays ? rays[r] : (int32_t)r;
+        const int32_t u = pix % Wd, v = pix / Wd;
+        const float uc = (float)u + 0.5f, vc = (float)v + 0.5f;
+        for (int k = 0; k < n_views; ++k)
+            for (int a = 0; a < 3; ++a)
+                b[k][a] = fmaf(Hm[k][3 * a + 0], uc, fmaf(Hm[k][3 * a + 1], vc, Hm[k][3 * a + 2]));
+        const OrcRayEval E = {n_views, views, maps, b, ev, tau};
+        float z = z_near, za = 0.0f, zb = 0.0f, Wb = 0.0f;
+        bool prev_pos = false, hit = false;
+        int32_t n = 0;
+        while (n < max_evals && !(z > z_far)) {                   // M1
+            float A, Wn;
+            orc_eval_s(E, z, &A, &Wn);
+            ++n;
+            float step;
+            if (Wn > 0.0f) {
+                const float s = A / Wn;
+                if (s > 0.0f) {
+                    za = z; prev_pos = true;
+                    step = fmaxf(step_scale * s, min_step);       // M2
+                } else {
+                    if (prev_pos) { zb = z; Wb = Wn; hit = true; break; }   // M4: change of sign
+                    step = min_step;
+                }
+            } else {
+                prev_pos = false;
+                step = free_step;                                 // M3
+            }
+            z = z + step;
+        }
+        float d = 0.0f, c = 0.0f;
+        if (hit) {
+            for (int i = 0; i < n_bisect; ++i) {                  // M5
+                const float m = 0.5f * (za + zb);
+                float A, Wn;
+                orc_eval_s(E, m, &A, &Wn);
+                ++n;
+                if (!(Wn > 0.0f)) break;
+                const float s = A / Wn;
+                if (s > 0.0f) za = m; else { zb = m; Wb = Wn; }
+            }
+            d = 0.5f * (za + zb);
+            c = Wb;                                               // M6
+        }
+        if (depth) depth[r] = d;
+        if (conf) conf[r] = c;
+        if (steps) steps[r] = n;
+    }
+    delete[] Hm; delete[] ev; delete[] b;
+    return 0;
+}
