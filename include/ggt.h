@@ -8,6 +8,8 @@
  *                      the target view's image space (pixel u,v x depth bin), overwrite or persistent
  *                      (Eq. 9-12; persistence: analogue of Eq. 13-14)
  *   ggt_extract_depth  volume -> per-pixel zero-crossing depth + confidence
+ * plus ggt_raymarch_depth, the paper's own volume-free schedule (adaptive advance 0.8 s, sign change, three
+ * bisection steps: PAPER.md:75, 348) on the same inputs.
  *
  * Conventions
  *   - every call returns int: GGT_OK (0) or a negative GGT_ERR_*; ggt_last_error() gives the text.
@@ -92,8 +94,9 @@ int64_t ggt_launch_count(const ggt_ctx* ctx);
 
 /* Optional per-stage device timing for bench.py's roofline: when enabled, every call records a pair of
  * CUDA events on the caller's stream around its kernels.  ggt_profile_collect waits for them, writes the
- * summed milliseconds and the number of timed groups per stage into host arrays of 4 entries
- * (0 refine, 1 weight maps, 2 integrate main kernel, 3 extract) and clears the records. */
+ * summed milliseconds and the number of timed groups per stage into host arrays of GGT_PROFILE_STAGES entries
+ * (0 refine, 1 weight maps, 2 integrate main kernel, 3 extract, 4 raymarch kernel) and clears the records. */
+#define GGT_PROFILE_STAGES 5
 int ggt_profile_enable(ggt_ctx* ctx, int32_t enable);
 int ggt_profile_collect(ggt_ctx* ctx, double* host_ms, int64_t* host_count);
 
@@ -157,6 +160,40 @@ int ggt_extract_depth(ggt_ctx* ctx, const ggt_volume* vol, float* dev_depth, flo
 int ggt_integrate_extract(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
                           const ggt_camera* views, const float* const* dev_depths, uint32_t flags,
                           float* dev_depth, float* dev_conf, int32_t* dev_bin, void* stream);
+
+/* ---- the paper's own schedule: volume-free adaptive raymarch ----------------- */
+/* PAPER.md:75 "integrates depth along each ray on the fly and, thus, avoids creating an explicit 3D voxel
+ * grid"; "We advance along the ray with a step size of 0.8s until a surface intersection is
+ * detected.  This is indicated by a change of sign in the value of s.  We subsequently perform three steps
+ * of a bisection search to refine the intersection depth."  s(z) is Eq. 9-10 (signs / normalisation:
+ * readings P1, P2) with the metric truncation `tau` (paper: 0.02 m) and the weights of Eq. 11-12, evaluated
+ * on the fly at target z-depth z; no ggt_volume is involved.  Readings M1-M6:
+ *   start at z_near; miss once z > z_far or after max_evals evaluations; advance max(step_scale * s,
+ *   min_step) after a positive sample, max(step_scale * tau, min_step) after an unobserved one, min_step
+ *   after a non-positive one that has no observed positive predecessor; a crossing is a sample s <= 0 whose
+ *   previous sample was observed and positive; n_bisect bisection steps (an unobserved midpoint ends them);
+ *   depth = midpoint of the final bracket; conf = sum of weights at its far end; steps = evaluations of s.
+ * Paper values: tau 0.02, step_scale 0.8, n_bisect 3, w_sigma0 0.001, w_clip 0.02, w_window 7; min_step and
+ * max_evals are this library's (defaults used by the binding: 1e-3 m, 4096). */
+typedef struct ggt_raymarch_params {
+    float z_near, z_far;           /* metres, z_far > z_near */
+    float tau;                     /* > 0 */
+    float step_scale;              /* > 0 */
+    float min_step;                /* > 0 */
+    int32_t max_evals;             /* >= 1 */
+    int32_t n_bisect;              /* >= 0 */
+    float w_sigma0, w_clip;
+    int32_t w_window;              /* 0 or 7 */
+} ggt_raymarch_params;
+
+/* target, views: HOST.  dev_depths: HOST array of n_views DEVICE pointers (fp32 height x width z-depth,
+ * <= 0 invalid).  Outputs: DEVICE, target->height x target->width, fp32 depth (0 = miss), fp32 conf
+ * (0 = miss), int32 steps; any may be NULL.  Uses the context's {depth, omega} workspace like
+ * ggt_integrate.  Errors: GGT_ERR_INVALID_ARG (NULLs, parameter ranges), GGT_ERR_SHAPE (sizes, n_views),
+ * GGT_ERR_UNSUPPORTED (w_window), GGT_ERR_CUDA. */
+int ggt_raymarch_depth(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views, const ggt_camera* views,
+                       const float* const* dev_depths, const ggt_raymarch_params* params, float* dev_depth,
+                       float* dev_conf, int32_t* dev_steps, void* stream);
 
 /* ---- end-to-end frame from HOST buffers (bench.py "e2e") ----------------------------------------- */
 /* One whole frame through the three steps with host<->device copies inside the call, all enqueued on

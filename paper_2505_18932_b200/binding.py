@@ -19,12 +19,13 @@ GGT_OK = 0
 GGT_F32, GGT_F16 = 0, 1
 GGT_OVERWRITE, GGT_ACCUMULATE = 0, 1
 GGT_MAX_VIEWS = 16
+GGT_PROFILE_STAGES = 5
 
 EXPORTS = [
     "ggt_create", "ggt_destroy", "ggt_last_error", "ggt_launch_count", "ggt_profile_enable", "ggt_profile_collect", "ggt_selftest_arith", "ggt_workspace_bytes", "ggt_set_workspace",
     "ggt_volume_bytes", "ggt_volume_bind", "ggt_volume_unbind", "ggt_volume_reset", "ggt_volume_export",
     "ggt_volume_tables", "ggt_refine_depth", "ggt_integrate", "ggt_extract_depth", "ggt_integrate_extract",
-    "ggt_frame_staging_bytes", "ggt_frame_host",
+    "ggt_raymarch_depth", "ggt_frame_staging_bytes", "ggt_frame_host",
 ]
 
 
@@ -41,6 +42,13 @@ class ggt_camera(ctypes.Structure):
 class ggt_refine_params(ctypes.Structure):
     _fields_ = [("lambda_t", ctypes.c_float), ("beta", ctypes.c_float), ("theta", ctypes.c_float),
                 ("downscale", ctypes.c_int32), ("pool", ctypes.c_int32)]
+
+
+class ggt_raymarch_params(ctypes.Structure):
+    _fields_ = [("z_near", ctypes.c_float), ("z_far", ctypes.c_float), ("tau", ctypes.c_float),
+                ("step_scale", ctypes.c_float), ("min_step", ctypes.c_float), ("max_evals", ctypes.c_int32),
+                ("n_bisect", ctypes.c_int32), ("w_sigma0", ctypes.c_float), ("w_clip", ctypes.c_float),
+                ("w_window", ctypes.c_int32)]
 
 
 class ggt_volume_desc(ctypes.Structure):
@@ -88,6 +96,8 @@ def load_library() -> ctypes.CDLL:
     lib.ggt_integrate.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), u32, vp]
     lib.ggt_extract_depth.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.ggt_integrate_extract.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), u32, vp, vp, vp, vp]
+    lib.ggt_raymarch_depth.argtypes = [vp, camp, i32, camp, ctypes.POINTER(vp), ctypes.POINTER(ggt_raymarch_params), vp, vp,
+                                       vp, vp]
     lib.ggt_frame_staging_bytes.argtypes = [descp, i32, i32, i32, i32]
     lib.ggt_frame_staging_bytes.restype = ctypes.c_size_t
     lib.ggt_frame_host.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), ctypes.POINTER(vp),
@@ -159,10 +169,10 @@ class Context:
 
     def ggt_profile_collect(self):
         """{stage: (total ms, groups)} for refine / weight / integrate / extract since the last collect."""
-        ms = (ctypes.c_double * 4)()
-        n = (ctypes.c_int64 * 4)()
+        ms = (ctypes.c_double * GGT_PROFILE_STAGES)()
+        n = (ctypes.c_int64 * GGT_PROFILE_STAGES)()
         self.check(self.lib.ggt_profile_collect(self.h, ms, n), "ggt_profile_collect")
-        return {k: (ms[i], int(n[i])) for i, k in enumerate(("refine", "weight", "integrate", "extract"))}
+        return {k: (ms[i], int(n[i])) for i, k in enumerate(("refine", "weight", "integrate", "extract", "raymarch"))}
 
     def ggt_selftest_arith(self, a, b):
         """(reciprocal mismatches, division mismatches) of the kernel's arithmetic vs IEEE on cuda tensors a, b."""
@@ -227,6 +237,18 @@ class Context:
     def ggt_extract_depth(self, vol: "Volume", depth=None, conf=None, bins=None):
         rc = self.lib.ggt_extract_depth(self.h, vol.h, _ptr(depth), _ptr(conf), _ptr(bins), _stream())
         self.check(rc, "ggt_extract_depth")
+
+    # ---- f-1: the paper's own volume-free schedule ----------------------------------------------------
+    def ggt_raymarch_depth(self, target, views, depths, z_near, z_far, depth=None, conf=None, steps=None, tau=0.02,
+                           step_scale=0.8, min_step=1e-3, max_evals=4096, n_bisect=3, w_sigma0=0.001, w_clip=0.02,
+                           w_window=7):
+        V = len(views)
+        t, arr = self._cams(target, views)
+        ptrs = (ctypes.c_void_p * V)(*[d.data_ptr() for d in depths])
+        prm = ggt_raymarch_params(z_near, z_far, tau, step_scale, min_step, max_evals, n_bisect, w_sigma0, w_clip, w_window)
+        rc = self.lib.ggt_raymarch_depth(self.h, ctypes.byref(t), V, arr, ptrs, ctypes.byref(prm), _ptr(depth), _ptr(conf),
+                                         _ptr(steps), _stream())
+        self.check(rc, "ggt_raymarch_depth")
 
     # ---- end-to-end from host buffers -----------------------------------------------------------------
     def ggt_frame_host(self, vol: "Volume", target, views, host_rgb: Optional[Sequence], host_depth_in: Sequence,

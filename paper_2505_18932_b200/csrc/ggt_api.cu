@@ -304,18 +304,11 @@ int ggt_refine_depth(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t*
     return GGT_OK;
 }
 
-// Shared front end of ggt_integrate / ggt_integrate_extract: validation, workspace, weight maps, launch.
-static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
-                          const ggt_camera* views, const float* const* dev_depths, uint32_t flags, bool fused,
-                          float* dev_depth, float* dev_conf, int32_t* dev_bin, void* stream) {
-    if (!ctx) return GGT_ERR_INVALID_ARG;
-    if (!vol || !target || !views || !dev_depths) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL volume / camera / depth pointer");
-    if (n_views < 1 || n_views > GGT_MAX_VIEWS) return fail(ctx, GGT_ERR_SHAPE, "n_views %d not in [1, %d]", n_views, GGT_MAX_VIEWS);
-    if (flags != GGT_OVERWRITE && flags != GGT_ACCUMULATE) return fail(ctx, GGT_ERR_INVALID_ARG, "flags %u", flags);
-    if (target->width != vol->desc.width || target->height != vol->desc.height)
-        return fail(ctx, GGT_ERR_SHAPE, "target %dx%d does not match the volume %dx%d", target->width, target->height,
-                    vol->desc.width, vol->desc.height);
-    if (!(target->fx > 0.0f) || !(target->fy > 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "target focal length");
+// Shared by ggt_integrate and ggt_raymarch_depth: validates the views, sizes the {depth, omega} workspace, fills the
+// per-view kernel parameters (relative transform a4, map pointers) and launches the weight-map pre-pass (a3).
+static int prepare_views(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views, const ggt_camera* views,
+                         const float* const* dev_depths, float w_sigma0, float w_clip, int32_t w_window,
+                         GgtViewParams* vp, cudaStream_t st) {
     size_t need = 0;
     for (int k = 0; k < n_views; ++k) {
         if (views[k].width <= 0 || views[k].height <= 0 || views[k].width > 32767 || views[k].height > 32767)
@@ -331,6 +324,43 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
         if (e != cudaSuccess) return cuda_fail(ctx, e, "workspace allocation");
         ctx->ws_bytes = need; ctx->ws_owned = true;
     }
+    char* w = static_cast<char*>(ctx->ws);
+    StageTimer tm(ctx, GGT_STAGE_WEIGHT, st);
+    GgtWeightParams wp;
+    memset(&wp, 0, sizeof wp);
+    wp.n_views = n_views; wp.window = w_window;
+    wp.sigma0 = w_sigma0; wp.c2 = w_clip * w_clip;
+    for (int k = 0; k < n_views; ++k) {
+        float hm[9], ev[3];
+        relative_transform(*target, views[k], hm, ev);
+        for (int i = 0; i < 6; ++i) vp[k].nh[i] = -hm[i];
+        for (int i = 0; i < 3; ++i) vp[k].h2[i] = hm[6 + i];
+        vp[k].ne[0] = -ev[0]; vp[k].ne[1] = -ev[1]; vp[k].e2 = ev[2];
+        vp[k].map = reinterpret_cast<const float2*>(w);
+        vp[k].width = views[k].width; vp[k].height = views[k].height;
+        vp[k].stride = (uint32_t)views[k].width + 1u;
+        wp.v[k].depth = dev_depths[k]; wp.v[k].out = reinterpret_cast<float2*>(w);
+        wp.v[k].width = views[k].width; wp.v[k].height = views[k].height;
+        w += align_up(((size_t)views[k].width + 1) * ((size_t)views[k].height + 1) * sizeof(float2), 256);
+    }
+    cudaError_t e = ggt_launch_weight_maps(wp, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "weight-map launch");
+    ctx->launches += 1;
+    return GGT_OK;
+}
+
+// Shared front end of ggt_integrate / ggt_integrate_extract: validation, workspace, weight maps, launch.
+static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
+                          const ggt_camera* views, const float* const* dev_depths, uint32_t flags, bool fused,
+                          float* dev_depth, float* dev_conf, int32_t* dev_bin, void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    if (!vol || !target || !views || !dev_depths) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL volume / camera / depth pointer");
+    if (n_views < 1 || n_views > GGT_MAX_VIEWS) return fail(ctx, GGT_ERR_SHAPE, "n_views %d not in [1, %d]", n_views, GGT_MAX_VIEWS);
+    if (flags != GGT_OVERWRITE && flags != GGT_ACCUMULATE) return fail(ctx, GGT_ERR_INVALID_ARG, "flags %u", flags);
+    if (target->width != vol->desc.width || target->height != vol->desc.height)
+        return fail(ctx, GGT_ERR_SHAPE, "target %dx%d does not match the volume %dx%d", target->width, target->height,
+                    vol->desc.width, vol->desc.height);
+    if (!(target->fx > 0.0f) || !(target->fy > 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "target focal length");
     cudaStream_t st = (cudaStream_t)stream;
     GgtIntegrateParams p;
     memset(&p, 0, sizeof p);
@@ -341,29 +371,10 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
     p.decay = vol->desc.decay; p.cap = vol->desc.weight_cap;
     p.tables = vol->dev_tables; p.voxels = vol->dev_voxels;
     p.depth = dev_depth; p.conf = dev_conf; p.bin = dev_bin;
-    char* w = static_cast<char*>(ctx->ws);
     {
-    StageTimer tm(ctx, GGT_STAGE_WEIGHT, st);
-    GgtWeightParams wp;
-    memset(&wp, 0, sizeof wp);
-    wp.n_views = n_views; wp.window = vol->desc.w_window;
-    wp.sigma0 = vol->desc.w_sigma0; wp.c2 = vol->desc.w_clip * vol->desc.w_clip;
-    for (int k = 0; k < n_views; ++k) {
-        float hm[9], ev[3];
-        relative_transform(*target, views[k], hm, ev);
-        for (int i = 0; i < 6; ++i) p.v[k].nh[i] = -hm[i];
-        for (int i = 0; i < 3; ++i) p.v[k].h2[i] = hm[6 + i];
-        p.v[k].ne[0] = -ev[0]; p.v[k].ne[1] = -ev[1]; p.v[k].e2 = ev[2];
-        p.v[k].map = reinterpret_cast<const float2*>(w);
-        p.v[k].width = views[k].width; p.v[k].height = views[k].height;
-        p.v[k].stride = (uint32_t)views[k].width + 1u;
-        wp.v[k].depth = dev_depths[k]; wp.v[k].out = reinterpret_cast<float2*>(w);
-        wp.v[k].width = views[k].width; wp.v[k].height = views[k].height;
-        w += align_up(((size_t)views[k].width + 1) * ((size_t)views[k].height + 1) * sizeof(float2), 256);
-    }
-    cudaError_t e = ggt_launch_weight_maps(wp, st);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "weight-map launch");
-    ctx->launches += 1;
+        const int rc = prepare_views(ctx, target, n_views, views, dev_depths, vol->desc.w_sigma0, vol->desc.w_clip,
+                                     vol->desc.w_window, p.v, st);
+        if (rc != GGT_OK) return rc;
     }
     StageTimer tm(ctx, GGT_STAGE_INTEGRATE, st);
     p.same_size = 1;
@@ -399,6 +410,37 @@ int ggt_extract_depth(ggt_ctx* ctx, const ggt_volume* vol, float* dev_depth, flo
     StageTimer tm(ctx, GGT_STAGE_EXTRACT, (cudaStream_t)stream);
     cudaError_t e = ggt_launch_extract(p, vol->desc.dtype, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "extract launch");
+    ctx->launches += 1;
+    return GGT_OK;
+}
+
+int ggt_raymarch_depth(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views, const ggt_camera* views,
+                       const float* const* dev_depths, const ggt_raymarch_params* params, float* dev_depth,
+                       float* dev_conf, int32_t* dev_steps, void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    if (!target || !views || !dev_depths || !params) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL camera / depth / params pointer");
+    if (n_views < 1 || n_views > GGT_MAX_VIEWS) return fail(ctx, GGT_ERR_SHAPE, "n_views %d not in [1, %d]", n_views, GGT_MAX_VIEWS);
+    if (target->width <= 0 || target->height <= 0) return fail(ctx, GGT_ERR_SHAPE, "target size %dx%d", target->width, target->height);
+    if (!(target->fx > 0.0f) || !(target->fy > 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "target focal length");
+    if (!(params->z_far > params->z_near) || !(params->z_near > 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "z_near / z_far");
+    if (!(params->tau > 0.0f) || !(params->step_scale > 0.0f) || !(params->min_step > 0.0f))
+        return fail(ctx, GGT_ERR_INVALID_ARG, "tau, step_scale and min_step must be > 0");
+    if (params->max_evals < 1 || params->n_bisect < 0) return fail(ctx, GGT_ERR_INVALID_ARG, "max_evals / n_bisect");
+    if (params->w_window != 0 && params->w_window != 7) return fail(ctx, GGT_ERR_UNSUPPORTED, "w_window %d (0 or 7)", params->w_window);
+    cudaStream_t st = (cudaStream_t)stream;
+    GgtRaymarchParams p;
+    memset(&p, 0, sizeof p);
+    p.Wt = target->width; p.Ht = target->height; p.n_views = n_views;
+    p.max_evals = params->max_evals; p.n_bisect = params->n_bisect;
+    p.z_near = params->z_near; p.z_far = params->z_far; p.tau = params->tau;
+    p.step_scale = params->step_scale; p.min_step = params->min_step;
+    p.depth = dev_depth; p.conf = dev_conf; p.steps = dev_steps;
+    const int rc = prepare_views(ctx, target, n_views, views, dev_depths, params->w_sigma0, params->w_clip,
+                                 params->w_window, p.v, st);
+    if (rc != GGT_OK) return rc;
+    StageTimer tm(ctx, GGT_STAGE_RAYMARCH, st);
+    cudaError_t e = ggt_launch_raymarch(p, st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "raymarch launch");
     ctx->launches += 1;
     return GGT_OK;
 }

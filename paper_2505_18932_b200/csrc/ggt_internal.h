@@ -37,6 +37,15 @@ struct GgtIntegrateParams {
     GgtViewParams v[GGT_MAX_VIEWS];
 };
 
+struct GgtRaymarchParams {  // the paper's own schedule: one thread per target ray, no volume
+    int32_t Wt, Ht, n_views, max_evals, n_bisect;
+    float z_near, z_far, tau, step_scale, min_step;
+    float* depth;          // outputs (each may be null)
+    float* conf;
+    int32_t* steps;
+    GgtViewParams v[GGT_MAX_VIEWS];
+};
+
 struct GgtWeightView {
     const float* depth;    // fp32 height x width, <= 0 (or NaN) = invalid
     float2* out;           // (height + 1) x (width + 1) records {depth, omega}
@@ -76,7 +85,7 @@ struct ggt_ctx {
     size_t prof_used = 0;
 };
 
-enum { GGT_STAGE_REFINE = 0, GGT_STAGE_WEIGHT = 1, GGT_STAGE_INTEGRATE = 2, GGT_STAGE_EXTRACT = 3, GGT_N_STAGES = 4 };
+enum { GGT_STAGE_REFINE = 0, GGT_STAGE_WEIGHT = 1, GGT_STAGE_INTEGRATE = 2, GGT_STAGE_EXTRACT = 3, GGT_STAGE_RAYMARCH = 4, GGT_N_STAGES = 5 };
 
 struct ggt_volume {
     ggt_volume_desc desc;
@@ -98,6 +107,7 @@ cudaError_t ggt_launch_refine(int W, int H, const uint8_t* rgb_cur, const uint8_
                               float theta, cudaStream_t st, int* n_launches);
 cudaError_t ggt_launch_weight_maps(const GgtWeightParams& p, cudaStream_t st);
 cudaError_t ggt_launch_integrate(const GgtIntegrateParams& p, int dtype, bool fused, cudaStream_t st);
+cudaError_t ggt_launch_raymarch(const GgtRaymarchParams& p, cudaStream_t st);
 cudaError_t ggt_launch_extract(const GgtExtractParams& p, int dtype, cudaStream_t st);
 cudaError_t ggt_launch_export(const GgtExtractParams& p, int dtype, float* T, float* W, cudaStream_t st);
 cudaError_t ggt_launch_selftest_arith(long long n, const float* a, const float* b, unsigned* mismatch, cudaStream_t st);

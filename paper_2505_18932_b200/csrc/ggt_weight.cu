@@ -18,18 +18,14 @@
 //     matches the oracle's `dd < c2 ? dd : c2` for every other input as well (inf, huge values);
 //   * all views of a call are one launch (blockIdx.z = view).
 #include "ggt_internal.h"
+#include "ggt_packed.cuh"
 
 namespace {
 
-typedef unsigned long long u64;
 constexpr int BW = 64, BH = 16, R = 3;
 constexpr int SW = 32 + 2 * R, SH = BH + 2 * R;   // 38 pairs x 22 rows
 
-__device__ __forceinline__ u64 pk(float lo, float hi) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
-__device__ __forceinline__ void upk(u64 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
 __device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 
 __device__ __forceinline__ float omega_of(float D0, float nu, float sigma0, int window) {
     if (!(D0 > 0.0f)) return 0.0f;
