@@ -373,6 +373,32 @@ def main():
            "d2h_bytes_per_step": host.d2h, "ms_per_step": red_e["ms"] / e2e_steps, "steps": e2e_steps,
            "api": "ggt_frame_host (pinned host buffers, stream synchronised every step)"}
 
+    # ---- extra legs (not the headline): fused integrate+extract, and the paper's own volume-free schedule ------
+    extra = {}
+    if rank == 0:
+        k = max(3, min(args.steps, 20))
+        depths = dev.state if wl.colour else dev.depth_in[1]
+        fused_fn = lambda: dev.ctx.ggt_integrate_extract(dev.vol, inp.target, inp.views, depths, dev.flags, dev.depth, dev.conf)
+        ms_f = timed(torch, None, fused_fn, k, 3) / k
+        extra["fused_integrate_extract"] = {"ms_per_call": ms_f, "includes": "weight maps + fused integrate/extract kernel (no volume re-read)",
+                                            "gvoxel_view_per_s": inp.vv_per_step / (ms_f / 1e3) / 1e9}
+        n_t = t.width * t.height
+        steps_out = torch.zeros(n_t, dtype=torch.int32, device="cuda")
+        zn, zf = float(wl.z_bins[0]), float(wl.z_bins[-1])
+        rm_fn = lambda: dev.ctx.ggt_raymarch_depth(inp.target, inp.views, depths, zn, zf, depth=dev.depth, conf=dev.conf, steps=steps_out)
+        dev.ctx.ggt_profile_enable(True)
+        ms_r = timed(torch, None, rm_fn, k, 3) / k
+        prof_r = dev.ctx.ggt_profile_collect()
+        dev.ctx.ggt_profile_enable(False)
+        evals = float(steps_out.sum().item())
+        k_ms = prof_r["raymarch"][0] / max(prof_r["raymarch"][1], 1)
+        extra["paper_schedule_raymarch"] = {
+            "call": "ggt_raymarch_depth (PAPER.md:75, 348: on-the-fly TSDF, advance 0.8 s, 3 bisection steps; tau 0.02 m, "
+                    "min_step 1e-3 m), same inputs as the step, no volume",
+            "ms_per_call": ms_r, "kernel_ms": k_ms, "evaluations_per_ray_mean": evals / n_t,
+            "gsample_view_per_s": evals * inp.V / (k_ms / 1e3) / 1e9 if k_ms > 0 else None,
+            "hit_fraction": float((dev.depth > 0).float().mean().item())}
+
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -384,7 +410,8 @@ def main():
                               "note": "per-step device time per stage (CUDA events on the launching stream)"},
                 "ms_per_1080p_target_frame": ms_per_step,
                 "integrate_gvoxel_view_per_s": inp.vv_per_step / (integ_ms / 1e3) / 1e9 if integ_ms > 0 else None,
-                "paper_context": "PAPER.md Table 4: TSDF stage 6 ms/frame at 1352x1014, K=4, GPU not stated"}
+                "paper_context": "PAPER.md Table 4: TSDF stage 6 ms/frame at 1352x1014, K=4, GPU not stated",
+                "extra": extra}
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(inp)
         print(json.dumps(line))

@@ -438,6 +438,9 @@ int ggt_raymarch_depth(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views, 
     const int rc = prepare_views(ctx, target, n_views, views, dev_depths, params->w_sigma0, params->w_clip,
                                  params->w_window, p.v, st);
     if (rc != GGT_OK) return rc;
+    p.shared_w = n_views >= 2;
+    for (int k = 1; k < n_views; ++k)
+        if (memcmp(p.v[k].h2, p.v[0].h2, sizeof p.v[0].h2) != 0 || memcmp(&p.v[k].e2, &p.v[0].e2, sizeof(float)) != 0) p.shared_w = 0;
     StageTimer tm(ctx, GGT_STAGE_RAYMARCH, st);
     cudaError_t e = ggt_launch_raymarch(p, st);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "raymarch launch");

@@ -39,6 +39,7 @@ struct GgtIntegrateParams {
 
 struct GgtRaymarchParams {  // the paper's own schedule: one thread per target ray, no volume
     int32_t Wt, Ht, n_views, max_evals, n_bisect;
+    int32_t shared_w;      // row 2 of H_k and e_k[2] bit-identical in all views (n_views >= 2)
     float z_near, z_far, tau, step_scale, min_step;
     float* depth;          // outputs (each may be null)
     float* conf;
