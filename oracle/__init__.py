@@ -196,3 +196,32 @@ def raymarch(target, views: Sequence, maps: Sequence[np.ndarray], z_near, z_far,
     if rc != 0:
         raise ValueError("orc_raymarch rc=%d" % rc)
     return depth, conf, steps
+
+
+def temporal_weight(prev_cam, prev_depth, prev_conf, views: Sequence, masks: Sequence[np.ndarray], beta=1.0, eta=15.0):
+    """O-T (Eq. 13-14). Returns the fp32 weight map of the previous output depth, shape of prev_depth."""
+    lib = _load()
+    H, W = int(prev_cam.height), int(prev_cam.width)
+    d = np.ascontiguousarray(prev_depth, dtype=np.float32).reshape(H, W)
+    c = np.ascontiguousarray(prev_conf, dtype=np.float32).reshape(H, W)
+    V = len(views)
+    cams = (OrcCamera * max(V, 1))(*[_cam(v) for v in views])
+    masks = [np.ascontiguousarray(m, dtype=np.float32) for m in masks]
+    ptrs = (ctypes.POINTER(ctypes.c_float) * max(V, 1))(*[_p(m, ctypes.c_float) for m in masks])
+    out = np.empty((H, W), dtype=np.float32)
+    t = _cam(prev_cam)
+    rc = lib.orc_temporal_weight(ctypes.byref(t), _p(d, ctypes.c_float), _p(c, ctypes.c_float), ctypes.c_int32(V),
+                                 cams, ptrs, ctypes.c_float(beta), ctypes.c_float(eta), _p(out, ctypes.c_float))
+    if rc != 0:
+        raise ValueError("orc_temporal_weight rc=%d" % rc)
+    return out
+
+
+def view_record(depth, weight) -> np.ndarray:
+    """Interleaved {depth, omega} map of a view whose weights are given (e.g. temporal_weight) instead of Eq. 11-12."""
+    depth = np.asarray(depth, dtype=np.float32)
+    out = np.zeros(depth.shape + (2,), dtype=np.float32)
+    ok = depth > 0
+    out[..., 0] = depth
+    out[..., 1] = np.where(ok, np.asarray(weight, dtype=np.float32).reshape(depth.shape), 0)
+    return out

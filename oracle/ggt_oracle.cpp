@@ -24,6 +24,8 @@
 //   348    omega_k = 0 if s_k < -tau; surface = change of sign of s         -> orc_integrate / orc_extract
 //   75, 348 the paper's own schedule: on-the-fly TSDF, advance 0.8 s, sign change,
 //          three bisection steps (no volume)                                 -> orc_raymarch
+//   92-96, 352-360 Eq. 3, 13-14: previous output depth as one more view with a
+//          mask-gated, capped accumulated weight                             -> orc_temporal_weight
 //   356-360 Eq. 13-14 accumulated temporal weight with cap (analogue: P9)   -> orc_integrate (accumulate)
 //
 // Pins (tests/test_oracle_pins.py, -m "not gpu"): T1 analytic planes/spheres, T2 coincident camera,
@@ -541,5 +543,63 @@ extern "C" int orc_raymarch(const OrcCamera* tgt, int32_t n_views, const OrcCame
         if (steps) steps[r] = n;
     }
     delete[] Hm; delete[] ev; delete[] b;
+    return 0;
+}
+
+// --------------------------------------------------------------------------------------------------
+// O-T  Temporal fusion weight of the previous output depth (Eq. 3,
+// PAPER.md:352-360 Eq. 13-14).  The rendered depth of the previous frame, D^{t-1}, enters the TSDF of frame t
+// as one more depth view with its own pose (the previous target camera) and the per-pixel weight
+//   omega_tmp^t = min(beta * omega_acc^t * max(1 - M^t, 0), eta)            (Eq. 13, eta = 15)
+//   omega_acc^t = omega_tmp^{t-1} + sum_k omega_k^{t-1}                      (Eq. 14)
+// omega_acc is the sum of ALL fusion weights at the previous frame's surface point, i.e. the confidence the
+// raymarch / extract of frame t-1 returned (readings M6 / P13) when D^{t-2} took part in that frame's sum.
+// M^t, the difference mask in the novel view: the paper forward-splats the K input masks M_k^t (Eq. 1) into the
+// novel view and takes the maximum; reading F1 restates that as a gather: the surface point of pixel (u, v) of
+// D^{t-1} is projected into every input view (A.1's projection, nearest pixel as P4) and M^t is the maximum of
+// M_k^t over the views it lands in (0 if none; occlusion is not tested).  Invalid depth or omega_acc <= 0 -> 0.
+//   prev: camera of D^{t-1};  masks[k]: fp32 height_k x width_k mask of view k (orc_refine's M).
+// --------------------------------------------------------------------------------------------------
+extern "C" int orc_temporal_weight(const OrcCamera* prev, const float* prev_depth, const float* prev_conf,
+                                   int32_t n_views, const OrcCamera* views, const float* const* masks,
+                                   float beta, float eta, float* weight_out) {
+    if (n_views < 0) return -1;
+    const int32_t Wd = prev->width, Hd = prev->height;
+    const int nv = n_views > 0 ? n_views : 1;
+    float (*Hm)[9] = new float[nv][9];
+    float (*ev)[3] = new float[nv][3];
+    for (int k = 0; k < n_views; ++k) orc_relative(prev, &views[k], Hm[k], ev[k]);
+    for (int32_t v = 0; v < Hd; ++v)
+        for (int32_t u = 0; u < Wd; ++u) {
+            const int64_t i = (int64_t)v * Wd + u;
+            const float d = prev_depth[i], acc = prev_conf[i];
+            float wt = 0.0f;
+            if (d > 0.0f && acc > 0.0f) {
+                const float uc = (float)u + 0.5f, vc = (float)v + 0.5f;
+                float Mmax = 0.0f;
+                for (int k = 0; k < n_views; ++k) {
+                    const float bx = fmaf(Hm[k][0], uc, fmaf(Hm[k][1], vc, Hm[k][2]));
+                    const float by = fmaf(Hm[k][3], uc, fmaf(Hm[k][4], vc, Hm[k][5]));
+                    const float bw = fmaf(Hm[k][6], uc, fmaf(Hm[k][7], vc, Hm[k][8]));
+                    const float x = fmaf(d, bx, ev[k][0]);
+                    const float y = fmaf(d, by, ev[k][1]);
+                    const float w = fmaf(d, bw, ev[k][2]);
+                    if (w < 1e-6f) continue;
+                    const float rcp = 1.0f / w;
+                    const float px = x * rcp, py = y * rcp;
+                    const float fxp = std::floor(px), fyp = std::floor(py);
+                    if (!(fxp >= 0.0f) || !(fyp >= 0.0f) || !(fxp < (float)views[k].width) ||
+                        !(fyp < (float)views[k].height)) continue;
+                    const float Mk = masks[k][(int64_t)(int)fyp * views[k].width + (int)fxp];
+                    if (Mk > Mmax) Mmax = Mk;
+                }
+                const float stat = fmaxf(1.0f - Mmax, 0.0f);         // max(1 - M^t, 0)
+                const float ba = beta * acc;
+                const float t = ba * stat;
+                wt = t < eta ? t : eta;                               // Eq. 13
+            }
+            weight_out[i] = wt;
+        }
+    delete[] Hm; delete[] ev;
     return 0;
 }
