@@ -195,6 +195,38 @@ int ggt_raymarch_depth(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views, 
                        const float* const* dev_depths, const ggt_raymarch_params* params, float* dev_depth,
                        float* dev_conf, int32_t* dev_steps, void* stream);
 
+/* ---- paper-style temporal fusion: the previous output depth as one more view ---- */
+/* PAPER.md:92-96 (Eq. 3): D^t = Raymarch(TSDF({D_k^t}, D^{t-1})); PAPER.md:352-360 (Eq. 13-14): D^{t-1} is fused
+ * with the weight  omega_tmp^t = min(beta * omega_acc^t * max(1 - M^t, 0), eta),  omega_acc^t = omega_tmp^{t-1} +
+ * sum_k omega_k^{t-1}  (eta = 15; beta "controls the relative contribution of previous frames").
+ * ggt_temporal_weight computes omega_tmp^t per pixel of D^{t-1}:
+ *   prev_target     HOST, the camera D^{t-1} was rendered from (its own pose: a moving target is handled)
+ *   dev_prev_depth  DEVICE fp32 H_p x W_p, the previous output depth (<= 0 = none)
+ *   dev_prev_conf   DEVICE fp32 H_p x W_p, omega_acc: the confidence the previous ggt_raymarch_depth* /
+ *                   ggt_extract_depth call returned (sum of all fusion weights at the surface point, Eq. 14)
+ *   views, dev_masks  the n_views input cameras (HOST) and their fp32 difference masks M_k^t of THIS frame
+ *                   (DEVICE, height_k x width_k: ggt_refine_depth's dev_mask_out); 0 <= n_views <= GGT_MAX_VIEWS
+ *   M^t (reading F1): the surface point of each pixel of D^{t-1} is projected into every input view (nearest
+ *                   pixel) and M^t is the maximum of M_k^t over the views it lands in (0 if none); occlusion is
+ *                   not tested.  The paper forward-splats the masks instead.
+ *   dev_weight_out  DEVICE fp32 H_p x W_p.
+ * The *_weighted calls are ggt_integrate / ggt_raymarch_depth with per-view given weights: dev_weights is a HOST
+ * array of n_views DEVICE pointers; entry k NULL -> Eq. 11-12 from the depth map as usual, else the fp32
+ * height_k x width_k weights of view k (>= 0) are used as its omega.  dev_weights itself may be NULL.
+ * One frame of Eq. 3: ggt_temporal_weight(prev camera, D^{t-1}, conf^{t-1}, ...) -> w; then
+ * ggt_raymarch_depth_weighted with views = {inputs..., prev camera}, depths = {..., D^{t-1}}, weights =
+ * {NULL..., w}; its dev_conf output is the next frame's omega_acc. */
+int ggt_temporal_weight(ggt_ctx* ctx, const ggt_camera* prev_target, const float* dev_prev_depth,
+                        const float* dev_prev_conf, int32_t n_views, const ggt_camera* views,
+                        const float* const* dev_masks, float beta, float eta, float* dev_weight_out, void* stream);
+int ggt_integrate_weighted(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
+                           const ggt_camera* views, const float* const* dev_depths, const float* const* dev_weights,
+                           uint32_t flags, void* stream);
+int ggt_raymarch_depth_weighted(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views, const ggt_camera* views,
+                                const float* const* dev_depths, const float* const* dev_weights,
+                                const ggt_raymarch_params* params, float* dev_depth, float* dev_conf,
+                                int32_t* dev_steps, void* stream);
+
 /* ---- end-to-end frame from HOST buffers (bench.py "e2e") ----------------------------------------- */
 /* One whole frame through the three steps with host<->device copies inside the call, all enqueued on
  * `stream` without synchronising.  All n_views views must have the same width x height.

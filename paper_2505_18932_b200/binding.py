@@ -25,7 +25,8 @@ EXPORTS = [
     "ggt_create", "ggt_destroy", "ggt_last_error", "ggt_launch_count", "ggt_profile_enable", "ggt_profile_collect", "ggt_selftest_arith", "ggt_workspace_bytes", "ggt_set_workspace",
     "ggt_volume_bytes", "ggt_volume_bind", "ggt_volume_unbind", "ggt_volume_reset", "ggt_volume_export",
     "ggt_volume_tables", "ggt_refine_depth", "ggt_integrate", "ggt_extract_depth", "ggt_integrate_extract",
-    "ggt_raymarch_depth", "ggt_frame_staging_bytes", "ggt_frame_host",
+    "ggt_raymarch_depth", "ggt_temporal_weight", "ggt_integrate_weighted", "ggt_raymarch_depth_weighted",
+    "ggt_frame_staging_bytes", "ggt_frame_host",
 ]
 
 
@@ -98,6 +99,11 @@ def load_library() -> ctypes.CDLL:
     lib.ggt_integrate_extract.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), u32, vp, vp, vp, vp]
     lib.ggt_raymarch_depth.argtypes = [vp, camp, i32, camp, ctypes.POINTER(vp), ctypes.POINTER(ggt_raymarch_params), vp, vp,
                                        vp, vp]
+    lib.ggt_raymarch_depth_weighted.argtypes = [vp, camp, i32, camp, ctypes.POINTER(vp), ctypes.POINTER(vp),
+                                                ctypes.POINTER(ggt_raymarch_params), vp, vp, vp, vp]
+    lib.ggt_integrate_weighted.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), ctypes.POINTER(vp), u32, vp]
+    lib.ggt_temporal_weight.argtypes = [vp, camp, vp, vp, i32, camp, ctypes.POINTER(vp), ctypes.c_float, ctypes.c_float,
+                                        vp, vp]
     lib.ggt_frame_staging_bytes.argtypes = [descp, i32, i32, i32, i32]
     lib.ggt_frame_staging_bytes.restype = ctypes.c_size_t
     lib.ggt_frame_host.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), ctypes.POINTER(vp),
@@ -249,6 +255,40 @@ class Context:
         rc = self.lib.ggt_raymarch_depth(self.h, ctypes.byref(t), V, arr, ptrs, ctypes.byref(prm), _ptr(depth), _ptr(conf),
                                          _ptr(steps), _stream())
         self.check(rc, "ggt_raymarch_depth")
+
+    # ---- f-2: the previous output depth as one more view (Eq. 3, 13-14) ------------------------------
+    def ggt_temporal_weight(self, prev_target, prev_depth, prev_conf, views, masks, weight_out, beta=1.0, eta=15.0):
+        V = len(views)
+        t, arr = self._cams(prev_target, views if V else [prev_target])
+        ptrs = (ctypes.c_void_p * max(V, 1))(*[m.data_ptr() for m in masks])
+        rc = self.lib.ggt_temporal_weight(self.h, ctypes.byref(t), prev_depth.data_ptr(), prev_conf.data_ptr(), V, arr, ptrs,
+                                          beta, eta, weight_out.data_ptr(), _stream())
+        self.check(rc, "ggt_temporal_weight")
+
+    @staticmethod
+    def _weight_ptrs(weights, V):
+        if weights is None:
+            return None
+        return (ctypes.c_void_p * V)(*[None if w is None else w.data_ptr() for w in weights])
+
+    def ggt_integrate_weighted(self, vol: "Volume", target, views, depths, weights, flags=GGT_OVERWRITE):
+        V = len(views)
+        t, arr = self._cams(target, views)
+        ptrs = (ctypes.c_void_p * V)(*[d.data_ptr() for d in depths])
+        rc = self.lib.ggt_integrate_weighted(self.h, vol.h, ctypes.byref(t), V, arr, ptrs, self._weight_ptrs(weights, V), flags,
+                                             _stream())
+        self.check(rc, "ggt_integrate_weighted")
+
+    def ggt_raymarch_depth_weighted(self, target, views, depths, weights, z_near, z_far, depth=None, conf=None, steps=None,
+                                    tau=0.02, step_scale=0.8, min_step=1e-3, max_evals=4096, n_bisect=3, w_sigma0=0.001,
+                                    w_clip=0.02, w_window=7):
+        V = len(views)
+        t, arr = self._cams(target, views)
+        ptrs = (ctypes.c_void_p * V)(*[d.data_ptr() for d in depths])
+        prm = ggt_raymarch_params(z_near, z_far, tau, step_scale, min_step, max_evals, n_bisect, w_sigma0, w_clip, w_window)
+        rc = self.lib.ggt_raymarch_depth_weighted(self.h, ctypes.byref(t), V, arr, ptrs, self._weight_ptrs(weights, V),
+                                                  ctypes.byref(prm), _ptr(depth), _ptr(conf), _ptr(steps), _stream())
+        self.check(rc, "ggt_raymarch_depth_weighted")
 
     # ---- end-to-end from host buffers -----------------------------------------------------------------
     def ggt_frame_host(self, vol: "Volume", target, views, host_rgb: Optional[Sequence], host_depth_in: Sequence,

@@ -307,7 +307,7 @@ int ggt_refine_depth(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t*
 // Shared by ggt_integrate and ggt_raymarch_depth: validates the views, sizes the {depth, omega} workspace, fills the
 // per-view kernel parameters (relative transform a4, map pointers) and launches the weight-map pre-pass (a3).
 static int prepare_views(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views, const ggt_camera* views,
-                         const float* const* dev_depths, float w_sigma0, float w_clip, int32_t w_window,
+                         const float* const* dev_depths, const float* const* dev_weights, float w_sigma0, float w_clip, int32_t w_window,
                          GgtViewParams* vp, cudaStream_t st) {
     size_t need = 0;
     for (int k = 0; k < n_views; ++k) {
@@ -340,6 +340,7 @@ static int prepare_views(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views
         vp[k].width = views[k].width; vp[k].height = views[k].height;
         vp[k].stride = (uint32_t)views[k].width + 1u;
         wp.v[k].depth = dev_depths[k]; wp.v[k].out = reinterpret_cast<float2*>(w);
+        wp.v[k].weight = dev_weights ? dev_weights[k] : nullptr;
         wp.v[k].width = views[k].width; wp.v[k].height = views[k].height;
         w += align_up(((size_t)views[k].width + 1) * ((size_t)views[k].height + 1) * sizeof(float2), 256);
     }
@@ -351,7 +352,8 @@ static int prepare_views(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views
 
 // Shared front end of ggt_integrate / ggt_integrate_extract: validation, workspace, weight maps, launch.
 static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
-                          const ggt_camera* views, const float* const* dev_depths, uint32_t flags, bool fused,
+                          const ggt_camera* views, const float* const* dev_depths, const float* const* dev_weights,
+                          uint32_t flags, bool fused,
                           float* dev_depth, float* dev_conf, int32_t* dev_bin, void* stream) {
     if (!ctx) return GGT_ERR_INVALID_ARG;
     if (!vol || !target || !views || !dev_depths) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL volume / camera / depth pointer");
@@ -372,7 +374,7 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
     p.tables = vol->dev_tables; p.voxels = vol->dev_voxels;
     p.depth = dev_depth; p.conf = dev_conf; p.bin = dev_bin;
     {
-        const int rc = prepare_views(ctx, target, n_views, views, dev_depths, vol->desc.w_sigma0, vol->desc.w_clip,
+        const int rc = prepare_views(ctx, target, n_views, views, dev_depths, dev_weights, vol->desc.w_sigma0, vol->desc.w_clip,
                                      vol->desc.w_window, p.v, st);
         if (rc != GGT_OK) return rc;
     }
@@ -392,13 +394,19 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
 
 int ggt_integrate(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
                   const ggt_camera* views, const float* const* dev_depths, uint32_t flags, void* stream) {
-    return integrate_impl(ctx, vol, target, n_views, views, dev_depths, flags, false, nullptr, nullptr, nullptr, stream);
+    return integrate_impl(ctx, vol, target, n_views, views, dev_depths, nullptr, flags, false, nullptr, nullptr, nullptr, stream);
+}
+
+int ggt_integrate_weighted(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
+                           const ggt_camera* views, const float* const* dev_depths, const float* const* dev_weights,
+                           uint32_t flags, void* stream) {
+    return integrate_impl(ctx, vol, target, n_views, views, dev_depths, dev_weights, flags, false, nullptr, nullptr, nullptr, stream);
 }
 
 int ggt_integrate_extract(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
                           const ggt_camera* views, const float* const* dev_depths, uint32_t flags,
                           float* dev_depth, float* dev_conf, int32_t* dev_bin, void* stream) {
-    return integrate_impl(ctx, vol, target, n_views, views, dev_depths, flags, true, dev_depth, dev_conf, dev_bin, stream);
+    return integrate_impl(ctx, vol, target, n_views, views, dev_depths, nullptr, flags, true, dev_depth, dev_conf, dev_bin, stream);
 }
 
 int ggt_extract_depth(ggt_ctx* ctx, const ggt_volume* vol, float* dev_depth, float* dev_conf, int32_t* dev_bin,
@@ -417,6 +425,14 @@ int ggt_extract_depth(ggt_ctx* ctx, const ggt_volume* vol, float* dev_depth, flo
 int ggt_raymarch_depth(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views, const ggt_camera* views,
                        const float* const* dev_depths, const ggt_raymarch_params* params, float* dev_depth,
                        float* dev_conf, int32_t* dev_steps, void* stream) {
+    return ggt_raymarch_depth_weighted(ctx, target, n_views, views, dev_depths, nullptr, params, dev_depth, dev_conf,
+                                       dev_steps, stream);
+}
+
+int ggt_raymarch_depth_weighted(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views, const ggt_camera* views,
+                                const float* const* dev_depths, const float* const* dev_weights,
+                                const ggt_raymarch_params* params, float* dev_depth, float* dev_conf,
+                                int32_t* dev_steps, void* stream) {
     if (!ctx) return GGT_ERR_INVALID_ARG;
     if (!target || !views || !dev_depths || !params) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL camera / depth / params pointer");
     if (n_views < 1 || n_views > GGT_MAX_VIEWS) return fail(ctx, GGT_ERR_SHAPE, "n_views %d not in [1, %d]", n_views, GGT_MAX_VIEWS);
@@ -435,7 +451,7 @@ int ggt_raymarch_depth(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views, 
     p.z_near = params->z_near; p.z_far = params->z_far; p.tau = params->tau;
     p.step_scale = params->step_scale; p.min_step = params->min_step;
     p.depth = dev_depth; p.conf = dev_conf; p.steps = dev_steps;
-    const int rc = prepare_views(ctx, target, n_views, views, dev_depths, params->w_sigma0, params->w_clip,
+    const int rc = prepare_views(ctx, target, n_views, views, dev_depths, dev_weights, params->w_sigma0, params->w_clip,
                                  params->w_window, p.v, st);
     if (rc != GGT_OK) return rc;
     p.shared_w = n_views >= 2;
@@ -444,6 +460,35 @@ int ggt_raymarch_depth(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views, 
     StageTimer tm(ctx, GGT_STAGE_RAYMARCH, st);
     cudaError_t e = ggt_launch_raymarch(p, st);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "raymarch launch");
+    ctx->launches += 1;
+    return GGT_OK;
+}
+
+int ggt_temporal_weight(ggt_ctx* ctx, const ggt_camera* prev_target, const float* dev_prev_depth,
+                        const float* dev_prev_conf, int32_t n_views, const ggt_camera* views,
+                        const float* const* dev_masks, float beta, float eta, float* dev_weight_out, void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    if (!prev_target || !dev_prev_depth || !dev_prev_conf || !dev_weight_out || (n_views > 0 && (!views || !dev_masks)))
+        return fail(ctx, GGT_ERR_INVALID_ARG, "NULL argument to ggt_temporal_weight");
+    if (n_views < 0 || n_views > GGT_MAX_VIEWS) return fail(ctx, GGT_ERR_SHAPE, "n_views %d not in [0, %d]", n_views, GGT_MAX_VIEWS);
+    if (prev_target->width <= 0 || prev_target->height <= 0) return fail(ctx, GGT_ERR_SHAPE, "previous target size");
+    if (!(prev_target->fx > 0.0f) || !(prev_target->fy > 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "previous target focal length");
+    if (!(beta >= 0.0f) || !(eta >= 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "beta and eta must be >= 0");
+    GgtTemporalParams p;
+    memset(&p, 0, sizeof p);
+    p.Wt = prev_target->width; p.Ht = prev_target->height; p.n_views = n_views;
+    p.beta = beta; p.eta = eta;
+    p.prev_depth = dev_prev_depth; p.prev_conf = dev_prev_conf; p.out = dev_weight_out;
+    for (int k = 0; k < n_views; ++k) {
+        if (views[k].width <= 0 || views[k].height <= 0 || views[k].width > 32767 || views[k].height > 32767)
+            return fail(ctx, GGT_ERR_SHAPE, "view %d size %dx%d", k, views[k].width, views[k].height);
+        if (!dev_masks[k]) return fail(ctx, GGT_ERR_INVALID_ARG, "dev_masks[%d] is NULL", k);
+        relative_transform(*prev_target, views[k], p.v[k].h, p.v[k].e);
+        p.v[k].mask = dev_masks[k];
+        p.v[k].width = views[k].width; p.v[k].height = views[k].height;
+    }
+    cudaError_t e = ggt_launch_temporal_weight(p, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "temporal-weight launch");
     ctx->launches += 1;
     return GGT_OK;
 }

@@ -47,8 +47,25 @@ struct GgtRaymarchParams {  // the paper's own schedule: one 
     GgtViewParams v[GGT_MAX_VIEWS];
 };
 
+struct GgtMaskView {        // ggt_temporal_weight: previous-target pixel/depth -> view k homogeneous pixel, and view k's mask
+    float h[9];            // H_k = K_k R_k R_p^T K_p^-1
+    float e[3];            // e_k = K_k (t_k - R_k R_p^T t_p)
+    const float* mask;     // fp32 height x width (Eq. 1's M_k^t)
+    int32_t width, height;
+};
+
+struct GgtTemporalParams {
+    int32_t Wt, Ht, n_views, pad_;
+    float beta, eta;
+    const float* prev_depth;
+    const float* prev_conf;
+    float* out;
+    GgtMaskView v[GGT_MAX_VIEWS];
+};
+
 struct GgtWeightView {
     const float* depth;    // fp32 height x width, <= 0 (or NaN) = invalid
+    const float* weight;   // null: omega from Eq. 11-12; else the view's given per-pixel weights (e.g. Eq. 13)
     float2* out;           // (height + 1) x (width + 1) records {depth, omega}
     int32_t width, height;
 };
@@ -108,6 +125,7 @@ cudaError_t ggt_launch_refine(int W, int H, const uint8_t* rgb_cur, const uint8_
                               float theta, cudaStream_t st, int* n_launches);
 cudaError_t ggt_launch_weight_maps(const GgtWeightParams& p, cudaStream_t st);
 cudaError_t ggt_launch_integrate(const GgtIntegrateParams& p, int dtype, bool fused, cudaStream_t st);
+cudaError_t ggt_launch_temporal_weight(const GgtTemporalParams& p, cudaStream_t st);
 cudaError_t ggt_launch_raymarch(const GgtRaymarchParams& p, cudaStream_t st);
 cudaError_t ggt_launch_extract(const GgtExtractParams& p, int dtype, cudaStream_t st);
 cudaError_t ggt_launch_export(const GgtExtractParams& p, int dtype, float* T, float* W, cudaStream_t st);

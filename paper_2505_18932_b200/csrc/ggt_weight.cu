@@ -16,7 +16,8 @@
 //   * invalid and out-of-image neighbours are stored in the tile as NaN: (D0 - NaN)^2 = NaN and min(NaN, c2) = c2
 //     (min.f32 returns the non-NaN operand), which is exactly "contributes clip^2" with no validity test, and it
 //     matches the oracle's `dd < c2 ? dd : c2` for every other input as well (inf, huge values);
-//   * all views of a call are one launch (blockIdx.z = view).
+//   * all views of a call are one launch (blockIdx.z = view); a view that brings its own per-pixel weights (the
+//     previous output depth with Eq. 13's weight, ggt_*_weighted) is only packed.
 #include "ggt_internal.h"
 #include "ggt_packed.cuh"
 
@@ -61,6 +62,19 @@ k_weight_map(const GgtWeightParams p) {
     const int x0 = blockIdx.x * BW, y0 = blockIdx.y * BH;
     if (x0 > W || y0 > H) return;                         // views of different sizes share one grid
     const float* __restrict__ depth = vw.depth;
+    if (vw.weight) {                                      // given weights: just pack {D, w} (and the zero padding)
+        for (int i = ty * 32 + tx; i < BW * BH; i += 256) {
+            const int x = x0 + i % BW, y = y0 + i / BW;
+            if (x > W || y > H) continue;
+            float2 rec = make_float2(0.0f, 0.0f);
+            if (x < W && y < H) {
+                const float g = __ldg(depth + (size_t)y * W + x);
+                if (g > 0.0f) rec = make_float2(g, __ldg(vw.weight + (size_t)y * W + x));
+            }
+            vw.out[(size_t)y * ((size_t)W + 1) + x] = rec;
+        }
+        return;
+    }
     for (int i = ty * 32 + tx; i < SW * SH; i += 256) {
         const int lx = i % SW, ly = i / SW;
         const int x = x0 - R + lx, y = y0 - R + ly;
