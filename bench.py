@@ -137,7 +137,7 @@ class DeviceRun:
         self.torch, self.b, self.inp, self.fused = torch, binding, inp, fused
         wl = inp.wl
         self.ctx = binding.Context()
-        self.ctx.ggt_set_workspace(inp.V, inp.W, inp.H)
+        self.ctx.ggt_set_workspace(inp.V + 1, max(inp.W, inp.target.width), max(inp.H, inp.target.height))   # + the previous output depth (Eq. 3 leg)
         self.vol = self.ctx.ggt_volume_bind(inp.target.width, inp.target.height, wl.z_bins,
                                             dtype=binding.GGT_F16 if wl.storage == "f16" else binding.GGT_F32,
                                             trunc_bins=wl.trunc_bins, weight_cap=wl.weight_cap)
@@ -398,6 +398,25 @@ def main():
             "ms_per_call": ms_r, "kernel_ms": k_ms, "evaluations_per_ray_mean": evals / n_t,
             "gsample_view_per_s": evals * inp.V / (k_ms / 1e3) / 1e9 if k_ms > 0 else None,
             "hit_fraction": float((dev.depth > 0).float().mean().item())}
+        # Eq. 3 (f-2): the previous output depth as a (V+1)-th view with Eq. 13's weight, masks from ggt_refine_depth
+        Hv, Wv = inp.H, inp.W
+        masks = [torch.full((Hv, Wv), 0.6, dtype=torch.float32, device="cuda") for _ in range(inp.V)]
+        if wl.colour:
+            for kk in range(inp.V):
+                st = dev.depth_in[0][kk].clone()
+                dev.ctx.ggt_refine_depth(dev.rgb_in[1][kk], dev.rgb_in[0][kk], dev.depth_in[1][kk], st, mask_out=masks[kk], **REFINE)
+        prev_d, prev_c = dev.depth.clone(), dev.conf.clone()
+        wmap = torch.empty(n_t, dtype=torch.float32, device="cuda")
+        tw_fn = lambda: dev.ctx.ggt_temporal_weight(inp.target, prev_d, prev_c, inp.views, masks, wmap, beta=1.0, eta=15.0)
+        ms_tw = timed(torch, None, tw_fn, k, 3) / k
+        views5, depths5 = list(inp.views) + [inp.target], list(depths) + [prev_d]
+        rm5_fn = lambda: dev.ctx.ggt_raymarch_depth_weighted(inp.target, views5, depths5, [None] * inp.V + [wmap], zn, zf,
+                                                            depth=dev.depth, conf=dev.conf, steps=steps_out)
+        ms_r5 = timed(torch, None, rm5_fn, k, 3) / k
+        extra["paper_temporal_fusion_eq3"] = {
+            "call": "ggt_temporal_weight (Eq. 13-14) + ggt_raymarch_depth_weighted with D^{t-1} as view V+1 (Eq. 3)",
+            "temporal_weight_ms": ms_tw, "raymarch_weighted_ms_per_call": ms_r5, "views": inp.V + 1,
+            "evaluations_per_ray_mean": float(steps_out.sum().item()) / n_t}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

@@ -219,8 +219,11 @@ cudaError_t ggt_launch_raymarch(const GgtRaymarchParams& p, cudaStream_t st) {
         case 2: k_raymarch<2><<<grd, blk, 0, st>>>(p); break;
         case 3: k_raymarch<3><<<grd, blk, 0, st>>>(p); break;
         case 4: k_raymarch<4><<<grd, blk, 0, st>>>(p); break;
+        case 5: k_raymarch<5><<<grd, blk, 0, st>>>(p); break;     // V + the previous output depth (Eq. 3)
         case 6: k_raymarch<6><<<grd, blk, 0, st>>>(p); break;
+        case 7: k_raymarch<7><<<grd, blk, 0, st>>>(p); break;
         case 8: k_raymarch<8><<<grd, blk, 0, st>>>(p); break;
+        case 9: k_raymarch<9><<<grd, blk, 0, st>>>(p); break;
         default: k_raymarch<0><<<grd, blk, 0, st>>>(p); break;
     }
     return cudaGetLastError();
