@@ -36,7 +36,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C3", choices=["C2", "C3", "C4"])
+    ap.add_argument("--workload", default="C3", choices=["C2", "C3", "C4", "C5"])
     ap.add_argument("--fused", action="store_true", help="use ggt_integrate_extract instead of integrate + extract")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -108,13 +108,20 @@ class Inputs:
         from paper_2505_18932_b200 import sharding, synth
         self.wl = wl = synth.workload(name)
         self.frames = sharding.frames_for_rank(rank, world, N_INPUT_FRAMES)
-        self.target = wl.targets(self.frames[0])[0]
-        self.vi = wl.views_for(self.target)
+        self.targets = wl.targets(self.frames[0])                  # C5: 8 targets per frame, else 1
+        self.vis = [wl.views_for(t) for t in self.targets]
+        self.target, self.vi = self.targets[0], self.vis[0]
         self.views = [wl.rig[v] for v in self.vi]
-        self.data = [[wl.view_inputs(f, v) for v in self.vi] for f in self.frames]   # [frame][view] -> (depth, rgb)
+        self.view_ids = sorted(set(v for vi in self.vis for v in vi))     # each rig view is refined once per frame
+        self.multi = len(self.targets) > 1
+        if self.multi:
+            self.data_by_view = [{v: wl.view_inputs(f, v) for v in self.view_ids} for f in self.frames]
+            self.data = [[d[v] for v in self.vi] for d in self.data_by_view]
+        else:
+            self.data = [[wl.view_inputs(f, v) for v in self.vi] for f in self.frames]   # [frame][view] -> (depth, rgb)
         self.W, self.H = self.views[0].width, self.views[0].height
         self.V = len(self.vi)
-        self.vv_per_step = float(self.target.width) * self.target.height * wl.z_bins.size * self.V
+        self.vv_per_step = float(sum(t.width * t.height * wl.z_bins.size * len(vi) for t, vi in zip(self.targets, self.vis)))
 
     def describe(self, world):
         wl, t = self.wl, self.target
@@ -122,7 +129,7 @@ class Inputs:
                             "of %dx%d from the 16-camera grid rig, %s %s volume, refine=%s"
                             % (wl.name, int(wl.name[1]) - 1, t.width, t.height, wl.z_bins.size, self.V, self.W, self.H,
                                wl.storage, "persistent" if wl.persistent else "overwrite", wl.colour),
-                "targets_per_step": 1, "views": self.V, "bins": int(wl.z_bins.size),
+                "targets_per_step": len(self.targets), "views": self.V, "bins": int(wl.z_bins.size),
                 "parallelism": "independent target streams per GPU x%d (no data-path collective)" % world,
                 "l2": "per-step traffic (volume %.2f GB written + read) exceeds the 126 MB L2; no explicit flush"
                       % (t.width * t.height * wl.z_bins.size * (4 if wl.storage == "f16" else 8) / 1e9)}
@@ -138,10 +145,19 @@ class DeviceRun:
         wl = inp.wl
         self.ctx = binding.Context()
         self.ctx.ggt_set_workspace(inp.V + 1, max(inp.W, inp.target.width), max(inp.H, inp.target.height))   # + the previous output depth (Eq. 3 leg)
-        self.vol = self.ctx.ggt_volume_bind(inp.target.width, inp.target.height, wl.z_bins,
-                                            dtype=binding.GGT_F16 if wl.storage == "f16" else binding.GGT_F32,
-                                            trunc_bins=wl.trunc_bins, weight_cap=wl.weight_cap)
-        self.vol.ggt_volume_reset()
+        self.vols = []
+        for t in inp.targets:
+            vol = self.ctx.ggt_volume_bind(t.width, t.height, wl.z_bins,
+                                           dtype=binding.GGT_F16 if wl.storage == "f16" else binding.GGT_F32,
+                                           trunc_bins=wl.trunc_bins, weight_cap=wl.weight_cap)
+            vol.ggt_volume_reset()
+            self.vols.append(vol)
+        self.vol = self.vols[0]
+        if inp.multi:          # [frame][rig view id] -> tensors; every view of the union is refined once per frame
+            self.depth_by = [{v: torch.from_numpy(np.array(d[v][0])).cuda() for v in inp.view_ids} for d in inp.data_by_view]
+            self.rgb_by = [{v: torch.from_numpy(np.array(d[v][1])).cuda() for v in inp.view_ids} for d in inp.data_by_view]
+            self.state_by = {v: self.depth_by[0][v].clone() for v in inp.view_ids}
+            self.tviews = [[wl.rig[v] for v in vi] for vi in inp.vis]
         self.depth_in = [[torch.from_numpy(np.array(d)).cuda() for d, _ in fr] for fr in inp.data]
         self.rgb_in = [[torch.from_numpy(np.array(r)).cuda() if r is not None else None for _, r in fr] for fr in inp.data]
         self.state = [self.depth_in[0][k].clone() for k in range(inp.V)]
@@ -156,6 +172,14 @@ class DeviceRun:
         cur = 1 + self.i % (N_INPUT_FRAMES - 1)
         prev = cur - 1
         self.i += 1
+        if inp.multi:
+            for v in inp.view_ids:
+                ctx.ggt_refine_depth(self.rgb_by[cur][v], self.rgb_by[prev][v], self.depth_by[cur][v], self.state_by[v], **REFINE)
+            for ti, t in enumerate(inp.targets):
+                depths = [self.state_by[v] for v in inp.vis[ti]]
+                ctx.ggt_integrate(self.vols[ti], t, self.tviews[ti], depths, self.flags)
+                ctx.ggt_extract_depth(self.vols[ti], self.depth, self.conf)
+            return
         if inp.wl.colour:
             for k in range(inp.V):
                 ctx.ggt_refine_depth(self.rgb_in[cur][k], self.rgb_in[prev][k], self.depth_in[cur][k], self.state[k], **REFINE)
@@ -314,7 +338,7 @@ def main():
 
     inp = Inputs(args.workload, rank, world)
     dev = DeviceRun(inp, args.fused)
-    host = HostRun(inp, dev)
+    host = HostRun(inp, dev) if not inp.multi else None
     hbm_peak, peak_src, _ = measured_peaks()
 
     # ---- headline: device-resident inputs --------------------------------------------------------------
@@ -348,14 +372,14 @@ def main():
     integ_bytes = vox_bytes * (2 if wl.persistent else 1) + map_bytes      # algorithmic: DESIGN.md "Roofline"
     integ_ms = prof["integrate"][0] / max(prof["integrate"][1], 1)
     achieved = integ_bytes / (integ_ms / 1e3) / 1e9 if integ_ms > 0 else 0.0
-    path_bytes = integ_bytes + (0 if args.fused else vox_bytes) + 2 * t.width * t.height * 4
+    path_bytes = (integ_bytes + (0 if args.fused else vox_bytes) + 2 * t.width * t.height * 4) * len(inp.targets)
     path_ms = stage_ms["integrate"] + stage_ms["extract"]
     roofline = {"bound": "hbm", "kernel": "k_integrate (ggt_integrate main kernel)", "achieved": achieved, "peak": hbm_peak,
                 "unit": "GB/s", "frac": achieved / hbm_peak, "traffic": None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": integ_bytes, "ms_per_launch": integ_ms,
                 "integrate_plus_extract": {"bytes": path_bytes, "ms": path_ms,
                                            "frac": (path_bytes / (path_ms / 1e3) / 1e9 / hbm_peak) if path_ms > 0 else 0.0},
-                "alu": {"flop_per_voxel_view": 16, "achieved_tflops": 16 * inp.vv_per_step / (integ_ms / 1e3) / 1e12 if integ_ms > 0 else 0.0,
+                "alu": {"flop_per_voxel_view": 16, "achieved_tflops": 16 * inp.vv_per_step / len(inp.targets) / (integ_ms / 1e3) / 1e12 if integ_ms > 0 else 0.0,
                         "peak_tflops_at_max_clock": 148 * 128 * 2 * 1.965e9 / 1e12}}
     traffic_file = os.path.join(ROOT, "profiles", "traffic_integrate.json")
     if os.path.exists(traffic_file):
@@ -363,19 +387,22 @@ def main():
             roofline["traffic"] = json.load(fh).get(wl.name + ("_fused" if args.fused else ""))
 
     # ---- e2e: host buffers through ggt_frame_host, result needed on the host every step ----------------
-    def e2e_step():
-        host.step()
-        torch.cuda.current_stream().synchronize()
-    e2e_steps = max(3, min(args.steps, 50))
-    ms_e2e_local = timed(torch, dist, e2e_step, e2e_steps, max(3, min(args.warmup, 5)))
-    red_e = sharding.reduce_timing(ms_e2e_local, inp.vv_per_step * e2e_steps, device="cuda" if dist is not None else None)
-    e2e = {"value": red_e["units"] / (red_e["ms"] / 1e3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": host.h2d,
-           "d2h_bytes_per_step": host.d2h, "ms_per_step": red_e["ms"] / e2e_steps, "steps": e2e_steps,
-           "api": "ggt_frame_host (pinned host buffers, stream synchronised every step)"}
+    if inp.multi:
+        e2e = {"value": None, "unit": UNIT, "note": "ggt_frame_host takes one target per call; the e2e leg runs on the single-target workloads (default C3)"}
+    else:
+        def e2e_step():
+            host.step()
+            torch.cuda.current_stream().synchronize()
+        e2e_steps = max(3, min(args.steps, 50))
+        ms_e2e_local = timed(torch, dist, e2e_step, e2e_steps, max(3, min(args.warmup, 5)))
+        red_e = sharding.reduce_timing(ms_e2e_local, inp.vv_per_step * e2e_steps, device="cuda" if dist is not None else None)
+        e2e = {"value": red_e["units"] / (red_e["ms"] / 1e3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": host.h2d,
+               "d2h_bytes_per_step": host.d2h, "ms_per_step": red_e["ms"] / e2e_steps, "steps": e2e_steps,
+               "api": "ggt_frame_host (pinned host buffers, stream synchronised every step)"}
 
     # ---- extra legs (not the headline): fused integrate+extract, and the paper's own volume-free schedule ------
     extra = {}
-    if rank == 0:
+    if rank == 0 and not inp.multi:
         k = max(3, min(args.steps, 20))
         depths = dev.state if wl.colour else dev.depth_in[1]
         fused_fn = lambda: dev.ctx.ggt_integrate_extract(dev.vol, inp.target, inp.views, depths, dev.flags, dev.depth, dev.conf)
@@ -428,10 +455,11 @@ def main():
                               "integrate": stage_ms["integrate"], "extract": stage_ms["extract"],
                               "note": "per-step device time per stage (CUDA events on the launching stream)"},
                 "ms_per_1080p_target_frame": ms_per_step,
-                "integrate_gvoxel_view_per_s": inp.vv_per_step / (integ_ms / 1e3) / 1e9 if integ_ms > 0 else None,
+                "integrate_gvoxel_view_per_s": inp.vv_per_step / len(inp.targets) / (integ_ms / 1e3) / 1e9 if integ_ms > 0 else None,
+                "ms_per_target": ms_per_step / len(inp.targets),
                 "paper_context": "PAPER.md Table 4: TSDF stage 6 ms/frame at 1352x1014, K=4, GPU not stated",
                 "extra": extra}
-        if not args.no_cpu_baseline and world == 1:
+        if not args.no_cpu_baseline and world == 1 and not inp.multi:
             line["cpu_baseline"] = cpu_baseline(inp)
         print(json.dumps(line))
     if dist is not None:
