@@ -225,3 +225,18 @@ def view_record(depth, weight) -> np.ndarray:
     out[..., 0] = depth
     out[..., 1] = np.where(ok, np.asarray(weight, dtype=np.float32).reshape(depth.shape), 0)
     return out
+
+
+def features(target, depth, views: Sequence) -> np.ndarray:
+    """O-F (PAPER.md:374-388 items 5-8). Returns (4 K, H, W) float32."""
+    lib = _load()
+    H, W = int(target.height), int(target.width)
+    d = np.ascontiguousarray(depth, dtype=np.float32).reshape(H, W)
+    V = len(views)
+    cams = (OrcCamera * max(V, 1))(*[_cam(v) for v in views])
+    out = np.empty((4 * V, H, W), dtype=np.float32)
+    t = _cam(target)
+    rc = lib.orc_features(ctypes.byref(t), _p(d, ctypes.c_float), ctypes.c_int32(V), cams, _p(out, ctypes.c_float))
+    if rc != 0:
+        raise ValueError("orc_features rc=%d" % rc)
+    return out

@@ -26,6 +26,8 @@
 //          three bisection steps (no volume)                                 -> orc_raymarch
 //   92-96, 352-360 Eq. 3, 13-14: previous output depth as one more view with a
 //          mask-gated, capped accumulated weight                             -> orc_temporal_weight
+//   374-388 A.4 items 5-8: ray / normal / view-direction dot products and camera
+//          distance maps of the guidance depth (network input features)     -> orc_features
 //   356-360 Eq. 13-14 accumulated temporal weight with cap (analogue: P9)   -> orc_integrate (accumulate)
 //
 // Pins (tests/test_oracle_pins.py, -m "not gpu"): T1 analytic planes/spheres, T2 coincident camera,
@@ -601,5 +603,121 @@ extern "C" int orc_temporal_weight(const OrcCamera* prev, const float* prev_dept
             weight_out[i] = wt;
         }
     delete[] Hm; delete[] ev;
+    return 0;
+}
+
+// --------------------------------------------------------------------------------------------------
+// O-F  Geometry features of the guidance depth for the blending network's input (
+// PAPER.md:374-388, items 5-8 of A.4: "the dot product between each input-view ray direction, and the normals from
+// the TSDF depth D^t", "the dot product between each input-view ray direction, and the target view direction",
+// "the distance between the input and target cameras, repeated spatially", "the dot product between the input and
+// target viewing directions, repeated spatially").  The paper gives no formulas; readings G1-G4:
+//   G1 the surface point of target pixel (u, v): p = D (( uc - cx)/fx, (vc - cy)/fy, 1) in the target camera,
+//      P = R_t^T (p - t_t) in the world;
+//   G2 normal: n_c = +-(dx x dy), dx = p(u+1, v) - p(u-1, v) where both neighbours have depth, else the one-sided
+//      difference with the neighbour that has, else undefined (same in v); oriented towards the camera (n_c . p <= 0),
+//      normalised; n = R_t^T n_c.  Undefined (or zero cross product) -> both per-pixel features are 0;
+//   G3 "input-view ray direction" at the pixel = unit vector from the input camera centre C_k = -R_k^T t_k to P;
+//      "target view direction" at the pixel = unit vector from C_t to P;
+//   G4 "viewing directions" = the cameras' optical axes (third rows of R); distance = |C_k - C_t|.
+// out: [4 K][H][W] fp32, planar: channels [0, K) item 5, [K, 2K) item 6, [2K, 3K) item 7, [3K, 4K) item 8.
+// --------------------------------------------------------------------------------------------------
+namespace {
+inline void orc_cam_point(const OrcCamera* c, const float* depth, int u, int v, float* p) {
+    const float d = depth[(int64_t)v * c->width + u];
+    const float uc = (float)u + 0.5f, vc = (float)v + 0.5f;
+    p[0] = d * ((uc - c->cx) / c->fx);
+    p[1] = d * ((vc - c->cy) / c->fy);
+    p[2] = d;
+}
+inline bool orc_has(const OrcCamera* c, const float* depth, int u, int v) {
+    return u >= 0 && v >= 0 && u < c->width && v < c->height && depth[(int64_t)v * c->width + u] > 0.0f;
+}
+// difference along one axis (du, dv): central, else one-sided, else false
+inline bool orc_diff(const OrcCamera* c, const float* depth, int u, int v, int du, int dv, float* out) {
+    const bool hp = orc_has(c, depth, u + du, v + dv), hm = orc_has(c, depth, u - du, v - dv);
+    float a[3], b[3];
+    if (hp && hm) { orc_cam_point(c, depth, u + du, v + dv, a); orc_cam_point(c, depth, u - du, v - dv, b); }
+    else if (hp) { orc_cam_point(c, depth, u + du, v + dv, a); orc_cam_point(c, depth, u, v, b); }
+    else if (hm) { orc_cam_point(c, depth, u, v, a); orc_cam_point(c, depth, u - du, v - dv, b); }
+    else return false;
+    for (int i = 0; i < 3; ++i) out[i] = a[i] - b[i];
+    return true;
+}
+inline float orc_dot(const float* a, const float* b) { return fmaf(a[2], b[2], fmaf(a[1], b[1], a[0] * b[0])); }
+// w = R^T q  (R row-major): w_i = R[0][i] q0 + R[1][i] q1 + R[2][i] q2
+inline void orc_rt_mul(const float* R, const float* q, float* w) {
+    for (int i = 0; i < 3; ++i) w[i] = fmaf(R[6 + i], q[2], fmaf(R[3 + i], q[1], R[i] * q[0]));
+}
+inline void orc_centre(const OrcCamera* c, float* C) {     // C = -R^T t, in double, rounded once
+    for (int i = 0; i < 3; ++i)
+        C[i] = (float)(-((double)c->R[i] * c->t[0] + (double)c->R[3 + i] * c->t[1] + (double)c->R[6 + i] * c->t[2]));
+}
+}  // namespace
+
+extern "C" int orc_features(const OrcCamera* tgt, const float* depth, int32_t n_views, const OrcCamera* views, float* out) {
+    if (n_views < 0) return -1;
+    const int32_t W = tgt->width, H = tgt->height;
+    const int64_t plane = (int64_t)W * H;
+    float Ct[3];
+    orc_centre(tgt, Ct);
+    float (*Ck)[3] = new float[n_views > 0 ? n_views : 1][3];
+    for (int k = 0; k < n_views; ++k) {
+        orc_centre(&views[k], Ck[k]);
+        const double dx = (double)Ck[k][0] - Ct[0], dy = (double)Ck[k][1] - Ct[1], dz = (double)Ck[k][2] - Ct[2];
+        const float dist = (float)std::sqrt(dx * dx + dy * dy + dz * dz);                              // item 7
+        const float axes = (float)((double)views[k].R[6] * tgt->R[6] + (double)views[k].R[7] * tgt->R[7] +
+                                   (double)views[k].R[8] * tgt->R[8]);                                 // item 8
+        for (int64_t i = 0; i < plane; ++i) {
+            out[(2 * n_views + k) * plane + i] = dist;
+            out[(3 * n_views + k) * plane + i] = axes;
+        }
+    }
+    for (int v = 0; v < H; ++v)
+        for (int u = 0; u < W; ++u) {
+            const int64_t i = (int64_t)v * W + u;
+            float n[3] = {0.0f, 0.0f, 0.0f}, P[3] = {0.0f, 0.0f, 0.0f};
+            bool ok = orc_has(tgt, depth, u, v);
+            if (ok) {
+                float p[3], dx[3], dy[3];
+                orc_cam_point(tgt, depth, u, v, p);
+                ok = orc_diff(tgt, depth, u, v, 1, 0, dx) && orc_diff(tgt, depth, u, v, 0, 1, dy);
+                if (ok) {
+                    float c[3] = {dx[1] * dy[2] - dx[2] * dy[1], dx[2] * dy[0] - dx[0] * dy[2], dx[0] * dy[1] - dx[1] * dy[0]};
+                    if (orc_dot(c, p) > 0.0f) { c[0] = -c[0]; c[1] = -c[1]; c[2] = -c[2]; }            // towards the camera
+                    const float l2 = orc_dot(c, c);
+                    ok = l2 > 0.0f;
+                    if (ok) {
+                        const float l = sqrtf(l2);
+                        const float nc[3] = {c[0] / l, c[1] / l, c[2] / l};
+                        orc_rt_mul(tgt->R, nc, n);
+                        const float q[3] = {p[0] - tgt->t[0], p[1] - tgt->t[1], p[2] - tgt->t[2]};
+                        orc_rt_mul(tgt->R, q, P);
+                    }
+                }
+            }
+            float rt[3] = {0.0f, 0.0f, 0.0f};
+            if (ok) {
+                const float d[3] = {P[0] - Ct[0], P[1] - Ct[1], P[2] - Ct[2]};
+                const float l = sqrtf(orc_dot(d, d));
+                ok = l > 0.0f;
+                if (ok) { rt[0] = d[0] / l; rt[1] = d[1] / l; rt[2] = d[2] / l; }
+            }
+            for (int k = 0; k < n_views; ++k) {
+                float f5 = 0.0f, f6 = 0.0f;
+                if (ok) {
+                    const float d[3] = {P[0] - Ck[k][0], P[1] - Ck[k][1], P[2] - Ck[k][2]};
+                    const float l = sqrtf(orc_dot(d, d));
+                    if (l > 0.0f) {
+                        const float rk[3] = {d[0] / l, d[1] / l, d[2] / l};
+                        f5 = orc_dot(rk, n);                                                            // item 5
+                        f6 = orc_dot(rk, rt);                                                           // item 6
+                    }
+                }
+                out[k * plane + i] = f5;
+                out[(n_views + k) * plane + i] = f6;
+            }
+        }
+    delete[] Ck;
     return 0;
 }
