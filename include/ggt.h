@@ -227,6 +227,23 @@ int ggt_raymarch_depth_weighted(ggt_ctx* ctx, const ggt_camera* target, int32_t 
                                 const ggt_raymarch_params* params, float* dev_depth, float* dev_conf,
                                 int32_t* dev_steps, void* stream);
 
+/* ---- network-input geometry features of the guidance depth --------------------- */
+/* PAPER.md:374-388 (A.4, items 5-8 of the blending network's input): per input view k and target pixel,
+ *   (5) the dot product between the input-view ray direction and the normal of the TSDF depth D^t,
+ *   (6) the dot product between the input-view ray direction and the target view direction,
+ *   (7) the distance between the input and target cameras, repeated spatially,
+ *   (8) the dot product between the input and target viewing directions, repeated spatially.
+ * Readings G1-G4: surface point p = D ((u + 0.5 - cx)/fx, (v + 0.5 - cy)/fy, 1) in the target camera;
+ * normal = normalised cross product of the central differences of p in u and v (one-sided where only one
+ * neighbour has depth, undefined where neither has), oriented towards the camera; ray directions are unit
+ * vectors from the camera centres -R^T t to the surface point; viewing directions are the optical axes.
+ *   target, views   HOST; 1 <= n_views <= GGT_MAX_VIEWS (only R, t of the views are used)
+ *   dev_depth       DEVICE fp32 H_t x W_t guidance depth (ggt_extract_depth / ggt_raymarch_depth output, <= 0 none)
+ *   dev_features    DEVICE fp32 [4 K][H_t][W_t], planar: channels [0, K) item 5, [K, 2K) item 6, [2K, 3K) item 7,
+ *                   [3K, 4K) item 8; items 5 and 6 are 0 where the depth or the normal is undefined. */
+int ggt_guidance_features(ggt_ctx* ctx, const ggt_camera* target, const float* dev_depth, int32_t n_views,
+                          const ggt_camera* views, float* dev_features, void* stream);
+
 /* ---- end-to-end frame from HOST buffers (bench.py "e2e") ----------------------------------------- */
 /* One whole frame through the three steps with host<->device copies inside the call, all enqueued on
  * `stream` without synchronising.  All n_views views must have the same width x height.

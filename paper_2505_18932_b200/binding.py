@@ -25,7 +25,7 @@ EXPORTS = [
     "ggt_create", "ggt_destroy", "ggt_last_error", "ggt_launch_count", "ggt_profile_enable", "ggt_profile_collect", "ggt_selftest_arith", "ggt_workspace_bytes", "ggt_set_workspace",
     "ggt_volume_bytes", "ggt_volume_bind", "ggt_volume_unbind", "ggt_volume_reset", "ggt_volume_export",
     "ggt_volume_tables", "ggt_refine_depth", "ggt_integrate", "ggt_extract_depth", "ggt_integrate_extract",
-    "ggt_raymarch_depth", "ggt_temporal_weight", "ggt_integrate_weighted", "ggt_raymarch_depth_weighted",
+    "ggt_raymarch_depth", "ggt_guidance_features", "ggt_temporal_weight", "ggt_integrate_weighted", "ggt_raymarch_depth_weighted",
     "ggt_frame_staging_bytes", "ggt_frame_host",
 ]
 
@@ -104,6 +104,7 @@ def load_library() -> ctypes.CDLL:
     lib.ggt_integrate_weighted.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), ctypes.POINTER(vp), u32, vp]
     lib.ggt_temporal_weight.argtypes = [vp, camp, vp, vp, i32, camp, ctypes.POINTER(vp), ctypes.c_float, ctypes.c_float,
                                         vp, vp]
+    lib.ggt_guidance_features.argtypes = [vp, camp, vp, i32, camp, vp, vp]
     lib.ggt_frame_staging_bytes.argtypes = [descp, i32, i32, i32, i32]
     lib.ggt_frame_staging_bytes.restype = ctypes.c_size_t
     lib.ggt_frame_host.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), ctypes.POINTER(vp),
@@ -289,6 +290,13 @@ class Context:
         rc = self.lib.ggt_raymarch_depth_weighted(self.h, ctypes.byref(t), V, arr, ptrs, self._weight_ptrs(weights, V),
                                                   ctypes.byref(prm), _ptr(depth), _ptr(conf), _ptr(steps), _stream())
         self.check(rc, "ggt_raymarch_depth_weighted")
+
+    # ---- f-4: network-input geometry features of the guidance depth ---------------------------------
+    def ggt_guidance_features(self, target, depth, views, features):
+        V = len(views)
+        t, arr = self._cams(target, views)
+        rc = self.lib.ggt_guidance_features(self.h, ctypes.byref(t), depth.data_ptr(), V, arr, features.data_ptr(), _stream())
+        self.check(rc, "ggt_guidance_features")
 
     # ---- end-to-end from host buffers -----------------------------------------------------------------
     def ggt_frame_host(self, vol: "Volume", target, views, host_rgb: Optional[Sequence], host_depth_in: Sequence,

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libggt.so")
-SOURCES = ["ggt_api.cu", "ggt_refine.cu", "ggt_weight.cu", "ggt_integrate.cu", "ggt_extract.cu", "ggt_raymarch.cu", "ggt_temporal.cu"]
+SOURCES = ["ggt_api.cu", "ggt_refine.cu", "ggt_weight.cu", "ggt_integrate.cu", "ggt_extract.cu", "ggt_raymarch.cu", "ggt_temporal.cu", "ggt_features.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--fmad=false", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math", "-shared", "-cudart", "shared"]
 

@@ -493,6 +493,41 @@ int ggt_temporal_weight(ggt_ctx* ctx, const ggt_camera* prev_target, const float
     return GGT_OK;
 }
 
+// camera centre C = -R^T t in double, rounded once (the oracle does the same)
+static void camera_centre(const ggt_camera& c, float* C) {
+    for (int i = 0; i < 3; ++i)
+        C[i] = (float)(-((double)c.R[i] * c.t[0] + (double)c.R[3 + i] * c.t[1] + (double)c.R[6 + i] * c.t[2]));
+}
+
+int ggt_guidance_features(ggt_ctx* ctx, const ggt_camera* target, const float* dev_depth, int32_t n_views,
+                          const ggt_camera* views, float* dev_features, void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    if (!target || !dev_depth || !dev_features || (n_views > 0 && !views))
+        return fail(ctx, GGT_ERR_INVALID_ARG, "NULL argument to ggt_guidance_features");
+    if (n_views < 1 || n_views > GGT_MAX_VIEWS) return fail(ctx, GGT_ERR_SHAPE, "n_views %d not in [1, %d]", n_views, GGT_MAX_VIEWS);
+    if (target->width <= 0 || target->height <= 0) return fail(ctx, GGT_ERR_SHAPE, "target size %dx%d", target->width, target->height);
+    if (!(target->fx > 0.0f) || !(target->fy > 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "target focal length");
+    GgtFeatureParams p;
+    memset(&p, 0, sizeof p);
+    p.W = target->width; p.H = target->height; p.n_views = n_views;
+    p.fx = target->fx; p.fy = target->fy; p.cx = target->cx; p.cy = target->cy;
+    for (int i = 0; i < 9; ++i) p.R[i] = target->R[i];
+    for (int i = 0; i < 3; ++i) p.t[i] = target->t[i];
+    camera_centre(*target, p.Ct);
+    p.depth = dev_depth; p.out = dev_features;
+    for (int k = 0; k < n_views; ++k) {
+        camera_centre(views[k], p.v[k].C);
+        const double dx = (double)p.v[k].C[0] - p.Ct[0], dy = (double)p.v[k].C[1] - p.Ct[1], dz = (double)p.v[k].C[2] - p.Ct[2];
+        p.v[k].dist = (float)std::sqrt(dx * dx + dy * dy + dz * dz);
+        p.v[k].axes = (float)((double)views[k].R[6] * target->R[6] + (double)views[k].R[7] * target->R[7] +
+                              (double)views[k].R[8] * target->R[8]);
+    }
+    cudaError_t e = ggt_launch_features(p, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "features launch");
+    ctx->launches += 1;
+    return GGT_OK;
+}
+
 // ---- end-to-end frame from host buffers -------------------------------------------------------------
 // staging layout (every block 256-B aligned), all views width x height:
 //   per slot s:  rgb[2][H*W*3] (ping-pong current / previous colour), state[H*W] fp32 refined depth

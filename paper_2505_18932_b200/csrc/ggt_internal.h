@@ -63,6 +63,21 @@ struct GgtTemporalParams {
     GgtMaskView v[GGT_MAX_VIEWS];
 };
 
+struct GgtFeatureView {
+    float C[3];            // camera centre -R_k^T t_k
+    float dist;            // |C_k - C_t|
+    float axes;            // optical axes: R_k row 2 . R_t row 2
+};
+
+struct GgtFeatureParams {   // ggt_guidance_features (A.4 items 5-8)
+    int32_t W, H, n_views, pad_;
+    float fx, fy, cx, cy;
+    float R[9], t[3], Ct[3];
+    const float* depth;
+    float* out;            // [4 K][H][W]
+    GgtFeatureView v[GGT_MAX_VIEWS];
+};
+
 struct GgtWeightView {
     const float* depth;    // fp32 height x width, <= 0 (or NaN) = invalid
     const float* weight;   // null: omega from Eq. 11-12; else the view's given per-pixel weights (e.g. Eq. 13)
@@ -126,6 +141,7 @@ cudaError_t ggt_launch_refine(int W, int H, const uint8_t* rgb_cur, const uint8_
 cudaError_t ggt_launch_weight_maps(const GgtWeightParams& p, cudaStream_t st);
 cudaError_t ggt_launch_integrate(const GgtIntegrateParams& p, int dtype, bool fused, cudaStream_t st);
 cudaError_t ggt_launch_temporal_weight(const GgtTemporalParams& p, cudaStream_t st);
+cudaError_t ggt_launch_features(const GgtFeatureParams& p, cudaStream_t st);
 cudaError_t ggt_launch_raymarch(const GgtRaymarchParams& p, cudaStream_t st);
 cudaError_t ggt_launch_extract(const GgtExtractParams& p, int dtype, cudaStream_t st);
 cudaError_t ggt_launch_export(const GgtExtractParams& p, int dtype, float* T, float* W, cudaStream_t st);
