@@ -425,6 +425,14 @@ def main():
             "ms_per_call": ms_r, "kernel_ms": k_ms, "evaluations_per_ray_mean": evals / n_t,
             "gsample_view_per_s": evals * inp.V / (k_ms / 1e3) / 1e9 if k_ms > 0 else None,
             "hit_fraction": float((dev.depth > 0).float().mean().item())}
+        # f-4: network-input geometry features of the guidance depth just produced
+        feats = torch.empty((4 * inp.V, t.height, t.width), dtype=torch.float32, device="cuda")
+        gdepth = dev.depth.clone()
+        ft_fn = lambda: dev.ctx.ggt_guidance_features(inp.target, gdepth, inp.views, feats)
+        ms_ft = timed(torch, None, ft_fn, k, 3) / k
+        ft_bytes = n_t * (4 + 16 * inp.V)
+        extra["guidance_features"] = {"call": "ggt_guidance_features (PAPER.md:374-388 items 5-8), [4K][H][W] fp32", "ms_per_call": ms_ft,
+                                      "algorithmic_bytes": ft_bytes, "frac_of_hbm_peak": ft_bytes / (ms_ft / 1e3) / 1e9 / hbm_peak}
         # Eq. 3 (f-2): the previous output depth as a (V+1)-th view with Eq. 13's weight, masks from ggt_refine_depth
         Hv, Wv = inp.H, inp.W
         masks = [torch.full((Hv, Wv), 0.6, dtype=torch.float32, device="cuda") for _ in range(inp.V)]
