@@ -245,8 +245,11 @@ int ggt_guidance_features(ggt_ctx* ctx, const ggt_camera* target, const float* d
                           const ggt_camera* views, float* dev_features, void* stream);
 
 /* ---- end-to-end frame from HOST buffers (bench.py "e2e") ----------------------------------------- */
-/* One whole frame through the three steps with host<->device copies inside the call, all enqueued on
- * `stream` without synchronising.  All n_views views must have the same width x height.
+/* One whole frame through the three steps with host<->device copies inside the call, enqueued without
+ * synchronising: kernels and the result copies on `stream`; the input uploads on a copy stream owned by the
+ * context, which `stream` waits for (events), so consecutive calls overlap frame n + 1's uploads with frame n's
+ * kernels.  The host input buffers must stay valid until `stream` has passed this call's kernels; the results
+ * are complete when `stream` is synchronised.  All n_views views must have the same width x height.
  *   host_rgb_cur[k]   uint8 HxWx3 colour of view k at this frame (host; array or entry may be NULL -> that
  *                     view is not refined, its depth is used as is); params NULL also disables refinement.
  *   host_depth_cur[k] fp32 HxW z-depth of view k (host).

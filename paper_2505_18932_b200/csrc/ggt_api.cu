@@ -131,6 +131,9 @@ int ggt_destroy(ggt_ctx* ctx) {
     if (c->ws_owned && c->ws) cudaFree(c->ws);
     if (c->cq) cudaFree(c->cq);
     for (auto& r : c->prof_pool) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    if (c->ev_inputs_free) cudaEventDestroy(c->ev_inputs_free);
+    if (c->ev_h2d_done) cudaEventDestroy(c->ev_h2d_done);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
     return GGT_OK;
 }
@@ -347,6 +350,11 @@ static int prepare_views(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views
     cudaError_t e = ggt_launch_weight_maps(wp, st);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "weight-map launch");
     ctx->launches += 1;
+    if (ctx->record_inputs_free) {     // ggt_frame_host: the uploaded inputs are dead from here on
+        e = cudaEventRecord(ctx->ev_inputs_free, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "event record");
+        ctx->inputs_free_pending = true;
+    }
     return GGT_OK;
 }
 
@@ -568,23 +576,51 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
     char* base = static_cast<char*>(dev_staging);
     char* view_base = base + (size_t)n_slots * (2 * rgb + dep);
     char* out_base = view_base + (size_t)n_views * dep;
+    // Uploads go to the context's copy stream, ordered after the previous frame's last reader of the input buffers
+    // (its weight-map pre-pass), so that they overlap that frame's integrate / extract when the caller does not
+    // synchronise in between; the caller's stream then waits for them.
+    if (!ctx->copy_stream) {
+        cudaError_t e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_inputs_free, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_h2d_done, cudaEventDisableTiming);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "copy stream / events");
+    }
+    cudaStream_t cs = ctx->copy_stream;
+    if (ctx->inputs_free_pending) {
+        cudaError_t e = cudaStreamWaitEvent(cs, ctx->ev_inputs_free, 0);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "stream wait");
+    }
     const float* dptr[GGT_MAX_VIEWS];
+    uint8_t* rcur[GGT_MAX_VIEWS];
+    const uint8_t* rprev[GGT_MAX_VIEWS];
+    for (int k = 0; k < n_views; ++k) {
+        char* slot = base + (size_t)slots[k] * (2 * rgb + dep);
+        float* dcur = reinterpret_cast<float*>(view_base + (size_t)k * dep);
+        cudaError_t e = cudaMemcpyAsync(dcur, host_depth_cur[k], px * 4, cudaMemcpyHostToDevice, cs);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D depth");
+        rcur[k] = nullptr; rprev[k] = nullptr;
+        if (refine && host_rgb_cur[k]) {
+            uint32_t& s = host_slot_state[slots[k]];          // bit 0: has history, bit 1: parity of "current"
+            const int cur = (s >> 1) & 1 ? 0 : 1;
+            rcur[k] = reinterpret_cast<uint8_t*>(slot + (size_t)cur * rgb);
+            rprev[k] = (s & 1) ? reinterpret_cast<const uint8_t*>(slot + (size_t)(1 - cur) * rgb) : nullptr;
+            e = cudaMemcpyAsync(rcur[k], host_rgb_cur[k], px * 3, cudaMemcpyHostToDevice, cs);
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D colour");
+            s = 1u | ((uint32_t)cur << 1);
+        }
+    }
+    {
+        cudaError_t e = cudaEventRecord(ctx->ev_h2d_done, cs);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ctx->ev_h2d_done, 0);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D event");
+    }
     for (int k = 0; k < n_views; ++k) {
         char* slot = base + (size_t)slots[k] * (2 * rgb + dep);
         float* state = reinterpret_cast<float*>(slot + 2 * rgb);
         float* dcur = reinterpret_cast<float*>(view_base + (size_t)k * dep);
-        cudaError_t e = cudaMemcpyAsync(dcur, host_depth_cur[k], px * 4, cudaMemcpyHostToDevice, st);
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D depth");
-        if (refine && host_rgb_cur[k]) {
-            uint32_t& s = host_slot_state[slots[k]];          // bit 0: has history, bit 1: parity of "current"
-            const int cur = (s >> 1) & 1 ? 0 : 1;
-            uint8_t* rc = reinterpret_cast<uint8_t*>(slot + (size_t)cur * rgb);
-            const uint8_t* rp = (s & 1) ? reinterpret_cast<const uint8_t*>(slot + (size_t)(1 - cur) * rgb) : nullptr;
-            e = cudaMemcpyAsync(rc, host_rgb_cur[k], px * 3, cudaMemcpyHostToDevice, st);
-            if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D colour");
-            int rcode = ggt_refine_depth(ctx, W, H, rc, rp, 3, dcur, state, nullptr, nullptr, params, stream);
+        if (rcur[k]) {
+            int rcode = ggt_refine_depth(ctx, W, H, rcur[k], rprev[k], 3, dcur, state, nullptr, nullptr, params, stream);
             if (rcode != GGT_OK) return rcode;
-            s = 1u | ((uint32_t)cur << 1);
             dptr[k] = state;
         } else {
             dptr[k] = dcur;
@@ -592,7 +628,9 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
     }
     float* d_depth = reinterpret_cast<float*>(out_base);
     float* d_conf = reinterpret_cast<float*>(out_base + out);
+    ctx->record_inputs_free = true;
     int rcode = ggt_integrate(ctx, vol, target, n_views, views, dptr, flags, stream);
+    ctx->record_inputs_free = false;
     if (rcode != GGT_OK) return rcode;
     rcode = ggt_extract_depth(ctx, vol, host_depth ? d_depth : nullptr, host_conf ? d_conf : nullptr, nullptr, stream);
     if (rcode != GGT_OK) return rcode;

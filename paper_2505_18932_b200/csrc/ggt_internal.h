@@ -111,6 +111,13 @@ struct ggt_ctx {
     bool ws_owned = false;
     uint16_t* cq = nullptr;        // quarter-res block differences of ggt_refine_depth (context-owned)
     size_t cq_bytes = 0;
+    // ggt_frame_host: host->device copies run on an internal stream so that the next frame's inputs upload while
+    // this frame's integrate / extract kernels run.  ev_inputs_free is recorded on the caller's stream once the
+    // weight-map pre-pass (the last kernel that reads the uploaded depth / colour buffers) has been enqueued.
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_inputs_free = nullptr, ev_h2d_done = nullptr;
+    bool inputs_free_pending = false;
+    bool record_inputs_free = false;
     // optional per-stage device timing (ggt_profile_enable): pairs of events around each kernel group
     bool prof = false;
     struct ProfRec { int stage; cudaEvent_t a, b; };

@@ -259,3 +259,36 @@ def test_frame_host_matches_device_path():
         torch.cuda.synchronize()
         assert torch.equal(hd, ref["depth"].cpu()) and torch.equal(hc, ref["conf"].cpu())
     assert (hd > 0).float().mean() > 0.5
+
+
+def test_frame_host_pipelined_without_host_sync():
+    """Frames enqueued back to back with no synchronise in between (ggt_frame_host uploads frame n + 1 on its own copy
+    stream while frame n computes) give, frame by frame, what the device-pointer calls give."""
+    import torch
+    from paper_2505_18932_b200 import binding
+    wl = synth.workload("C3", scale=0.25)
+    gp = helpers.CudaPipeline(wl)
+    ctx = binding.Context()
+    tgt = wl.targets(0)[0]
+    vi = wl.views_for(tgt)
+    views = [wl.rig[v] for v in vi]
+    H, W = views[0].height, views[0].width
+    vol = ctx.ggt_volume_bind(tgt.width, tgt.height, wl.z_bins)
+    n_slots = len(wl.rig)
+    nbytes = ctx.lib.ggt_frame_staging_bytes(ctypes.byref(vol.desc), n_slots, len(vi), W, H)
+    staging = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    state = np.zeros(n_slots, np.uint32)
+    prm = binding.ggt_refine_params(0.7, 0.6, 8.0 / 255.0, 4, 3)
+    F = 6
+    n = tgt.height * tgt.width
+    outs = [(torch.empty(n, dtype=torch.float32).pin_memory(), torch.empty(n, dtype=torch.float32).pin_memory()) for _ in range(F)]
+    ins = [[wl.view_inputs(f, v) for v in vi] for f in range(F)]
+    rgb = [[torch.from_numpy(r).pin_memory() for _, r in fr] for fr in ins]
+    dep = [[torch.from_numpy(d).pin_memory() for d, _ in fr] for fr in ins]
+    torch.cuda.synchronize()
+    for f in range(F):                                   # no synchronise inside the loop
+        ctx.ggt_frame_host(vol, tgt, views, rgb[f], dep[f], vi, state, staging, outs[f][0], outs[f][1], refine_params=prm)
+    torch.cuda.synchronize()
+    for f in range(F):
+        ref = gp.frame(f)[0]
+        assert torch.equal(outs[f][0], ref["depth"].cpu()) and torch.equal(outs[f][1], ref["conf"].cpu()), "frame %d" % f
