@@ -173,16 +173,16 @@ class DeviceRun:
         prev = cur - 1
         self.i += 1
         if inp.multi:
-            for v in inp.view_ids:
-                ctx.ggt_refine_depth(self.rgb_by[cur][v], self.rgb_by[prev][v], self.depth_by[cur][v], self.state_by[v], **REFINE)
+            ids = inp.view_ids
+            ctx.ggt_refine_depth_batch([self.rgb_by[cur][v] for v in ids], [self.rgb_by[prev][v] for v in ids],
+                                       [self.depth_by[cur][v] for v in ids], [self.state_by[v] for v in ids], **REFINE)
             for ti, t in enumerate(inp.targets):
                 depths = [self.state_by[v] for v in inp.vis[ti]]
                 ctx.ggt_integrate(self.vols[ti], t, self.tviews[ti], depths, self.flags)
                 ctx.ggt_extract_depth(self.vols[ti], self.depth, self.conf)
             return
         if inp.wl.colour:
-            for k in range(inp.V):
-                ctx.ggt_refine_depth(self.rgb_in[cur][k], self.rgb_in[prev][k], self.depth_in[cur][k], self.state[k], **REFINE)
+            ctx.ggt_refine_depth_batch(self.rgb_in[cur], self.rgb_in[prev], self.depth_in[cur], self.state, **REFINE)
             depths = self.state
         else:
             depths = self.depth_in[cur]

@@ -143,6 +143,16 @@ int ggt_refine_depth(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t*
                      float* dev_depth_state, float* dev_mask_out, uint16_t* dev_pooled_out,
                      const ggt_refine_params* params, void* stream);
 
+/* The same for n_views views of ONE size in two launches (a frame's views at once): every argument of
+ * ggt_refine_depth becomes a HOST array of n_views entries (device pointers).  dev_rgb_cur / dev_rgb_prev /
+ * dev_mask_out / dev_pooled_out may be NULL as arrays or per entry, with ggt_refine_depth's meaning (a view
+ * without dev_rgb_prev gets the first-frame rule).  1 <= n_views <= GGT_MAX_VIEWS. */
+int ggt_refine_depth_batch(ggt_ctx* ctx, int32_t n_views, int32_t width, int32_t height,
+                           const uint8_t* const* dev_rgb_cur, const uint8_t* const* dev_rgb_prev,
+                           int32_t rgb_pixel_stride, const float* const* dev_depth_cur, float* const* dev_depth_state,
+                           float* const* dev_mask_out, uint16_t* const* dev_pooled_out,
+                           const ggt_refine_params* params, void* stream);
+
 /* ---- steps a3-a6: fuse V depth maps into the target-view TSDF ----------------- */
 /* target, views: HOST.  dev_depths: HOST array of n_views DEVICE pointers to fp32 height x width
  * z-depth maps of the corresponding view (<= 0 invalid).  1 <= n_views <= GGT_MAX_VIEWS.

@@ -24,7 +24,7 @@ GGT_PROFILE_STAGES = 5
 EXPORTS = [
     "ggt_create", "ggt_destroy", "ggt_last_error", "ggt_launch_count", "ggt_profile_enable", "ggt_profile_collect", "ggt_selftest_arith", "ggt_workspace_bytes", "ggt_set_workspace",
     "ggt_volume_bytes", "ggt_volume_bind", "ggt_volume_unbind", "ggt_volume_reset", "ggt_volume_export",
-    "ggt_volume_tables", "ggt_refine_depth", "ggt_integrate", "ggt_extract_depth", "ggt_integrate_extract",
+    "ggt_volume_tables", "ggt_refine_depth", "ggt_refine_depth_batch", "ggt_integrate", "ggt_extract_depth", "ggt_integrate_extract",
     "ggt_raymarch_depth", "ggt_guidance_features", "ggt_temporal_weight", "ggt_integrate_weighted", "ggt_raymarch_depth_weighted",
     "ggt_frame_staging_bytes", "ggt_frame_host",
 ]
@@ -105,6 +105,9 @@ def load_library() -> ctypes.CDLL:
     lib.ggt_temporal_weight.argtypes = [vp, camp, vp, vp, i32, camp, ctypes.POINTER(vp), ctypes.c_float, ctypes.c_float,
                                         vp, vp]
     lib.ggt_guidance_features.argtypes = [vp, camp, vp, i32, camp, vp, vp]
+    lib.ggt_refine_depth_batch.argtypes = [vp, i32, i32, i32, ctypes.POINTER(vp), ctypes.POINTER(vp), i32, ctypes.POINTER(vp),
+                                           ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp),
+                                           ctypes.POINTER(ggt_refine_params), vp]
     lib.ggt_frame_staging_bytes.argtypes = [descp, i32, i32, i32, i32]
     lib.ggt_frame_staging_bytes.restype = ctypes.c_size_t
     lib.ggt_frame_host.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), ctypes.POINTER(vp),
@@ -209,6 +212,23 @@ class Context:
                                        _ptr(depth_state), _ptr(mask_out), _ptr(pooled_out), ctypes.byref(prm),
                                        _stream())
         self.check(rc, "ggt_refine_depth")
+
+    def ggt_refine_depth_batch(self, rgb_cur, rgb_prev, depth_cur, depth_state, mask_out=None, pooled_out=None,
+                               lambda_t=0.7, beta=0.6, theta=0.0, downscale=4, pool=3):
+        """ggt_refine_depth for a list of equally sized views in two launches; list entries may be None where allowed."""
+        V = len(depth_cur)
+        H, W = depth_cur[0].shape
+        first = next((r for r in (rgb_cur or []) if r is not None), None)
+        stride = 3 if first is None else int(first.shape[2])
+
+        def arr(lst):
+            if lst is None:
+                return None
+            return (ctypes.c_void_p * V)(*[None if t is None else t.data_ptr() for t in lst])
+        prm = _refine_params(lambda_t, beta, theta, downscale, pool)
+        rc = self.lib.ggt_refine_depth_batch(self.h, V, W, H, arr(rgb_cur), arr(rgb_prev), stride, arr(depth_cur),
+                                             arr(depth_state), arr(mask_out), arr(pooled_out), ctypes.byref(prm), _stream())
+        self.check(rc, "ggt_refine_depth_batch")
 
     # ---- volume ------------------------------------------------------------------------------------
     def ggt_volume_bind(self, width, height, z_bins, dtype=GGT_F32, trunc_bins=2.0, trunc_metric=0.0,

@@ -275,20 +275,35 @@ int ggt_volume_tables(const ggt_volume* vol, float* host_z, float* host_tau) {
     return GGT_OK;
 }
 
-int ggt_refine_depth(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t* dev_rgb_cur,
-                     const uint8_t* dev_rgb_prev, int32_t rgb_pixel_stride, const float* dev_depth_cur,
-                     float* dev_depth_state, float* dev_mask_out, uint16_t* dev_pooled_out,
-                     const ggt_refine_params* params, void* stream) {
+int ggt_refine_depth_batch(ggt_ctx* ctx, int32_t n_views, int32_t width, int32_t height,
+                           const uint8_t* const* dev_rgb_cur, const uint8_t* const* dev_rgb_prev,
+                           int32_t rgb_pixel_stride, const float* const* dev_depth_cur, float* const* dev_depth_state,
+                           float* const* dev_mask_out, uint16_t* const* dev_pooled_out,
+                           const ggt_refine_params* params, void* stream) {
     if (!ctx) return GGT_ERR_INVALID_ARG;
     ggt_ctx* c = ctx;
+    if (n_views < 1 || n_views > GGT_MAX_VIEWS) return fail(ctx, GGT_ERR_SHAPE, "n_views %d not in [1, %d]", n_views, GGT_MAX_VIEWS);
     if (width <= 0 || height <= 0) return fail(ctx, GGT_ERR_SHAPE, "image size %dx%d", width, height);
     if (!dev_depth_cur || !dev_depth_state || !params) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL depth / params pointer");
-    if (dev_rgb_prev && !dev_rgb_cur) return fail(ctx, GGT_ERR_INVALID_ARG, "rgb_prev given without rgb_cur");
     if (rgb_pixel_stride != 3 && rgb_pixel_stride != 4) return fail(ctx, GGT_ERR_INVALID_ARG, "rgb_pixel_stride %d (3 or 4)", rgb_pixel_stride);
     if (params->downscale != 4 || params->pool != 3) return fail(ctx, GGT_ERR_UNSUPPORTED, "only downscale 4 / pool 3 (PAPER.md:81) are implemented");
     if (!(params->lambda_t > 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "lambda_t must be > 0");
-    if (dev_rgb_prev) {
-        const size_t need = (size_t)((width + 3) / 4) * ((height + 3) / 4) * sizeof(uint16_t);
+    const size_t cq_one = align_up((size_t)((width + 3) / 4) * ((height + 3) / 4) * sizeof(uint16_t), 256);
+    GgtRefineViews tab;
+    memset(&tab, 0, sizeof tab);
+    for (int k = 0; k < n_views; ++k) {
+        if (!dev_depth_cur[k] || !dev_depth_state[k]) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL depth pointer of view %d", k);
+        const uint8_t* rc = dev_rgb_cur ? dev_rgb_cur[k] : nullptr;
+        const uint8_t* rp = dev_rgb_prev ? dev_rgb_prev[k] : nullptr;
+        if (rp && !rc) return fail(ctx, GGT_ERR_INVALID_ARG, "rgb_prev given without rgb_cur (view %d)", k);
+        if (!rp) continue;
+        GgtRefineView& v = tab.v[tab.n++];
+        v.rgb_cur = rc; v.rgb_prev = rp; v.depth_cur = dev_depth_cur[k]; v.depth_state = dev_depth_state[k];
+        v.mask_out = dev_mask_out ? dev_mask_out[k] : nullptr;
+        v.pooled_out = dev_pooled_out ? dev_pooled_out[k] : nullptr;
+    }
+    if (tab.n > 0) {
+        const size_t need = cq_one * tab.n;
         if (c->cq_bytes < need) {
             if (c->cq) cudaFree(c->cq);
             c->cq = nullptr; c->cq_bytes = 0;
@@ -296,15 +311,32 @@ int ggt_refine_depth(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t*
             if (e != cudaSuccess) return cuda_fail(ctx, e, "scratch for block differences");
             c->cq_bytes = need;
         }
+        for (int i = 0; i < tab.n; ++i) tab.v[i].cq = reinterpret_cast<uint16_t*>(reinterpret_cast<char*>(c->cq) + cq_one * i);
     }
-    int n = 0;
-    StageTimer tm(ctx, GGT_STAGE_REFINE, (cudaStream_t)stream);
-    cudaError_t e = ggt_launch_refine(width, height, dev_rgb_cur, dev_rgb_prev, rgb_pixel_stride, dev_depth_cur,
-                                      dev_depth_state, dev_mask_out, dev_pooled_out, c->cq, params->lambda_t,
-                                      params->beta, params->theta, (cudaStream_t)stream, &n);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "ggt_refine_depth launch");
-    ctx->launches += n;
+    cudaStream_t st = (cudaStream_t)stream;
+    StageTimer tm(ctx, GGT_STAGE_REFINE, st);
+    for (int k = 0; k < n_views; ++k) {                         // views without history: first-frame rule (M = 1)
+        if (dev_rgb_prev && dev_rgb_prev[k]) continue;
+        cudaError_t e = ggt_launch_first_frame(width, height, dev_depth_cur[k], dev_depth_state[k],
+                                               dev_mask_out ? dev_mask_out[k] : nullptr, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "ggt_refine_depth first-frame launch");
+        ctx->launches += 1;
+    }
+    if (tab.n > 0) {
+        int n = 0;
+        cudaError_t e = ggt_launch_refine(width, height, tab, rgb_pixel_stride, params->lambda_t, params->beta, params->theta, st, &n);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "ggt_refine_depth launch");
+        ctx->launches += n;
+    }
     return GGT_OK;
+}
+
+int ggt_refine_depth(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t* dev_rgb_cur,
+                     const uint8_t* dev_rgb_prev, int32_t rgb_pixel_stride, const float* dev_depth_cur,
+                     float* dev_depth_state, float* dev_mask_out, uint16_t* dev_pooled_out,
+                     const ggt_refine_params* params, void* stream) {
+    return ggt_refine_depth_batch(ctx, 1, width, height, &dev_rgb_cur, &dev_rgb_prev, rgb_pixel_stride, &dev_depth_cur,
+                                  &dev_depth_state, &dev_mask_out, &dev_pooled_out, params, stream);
 }
 
 // Shared by ggt_integrate and ggt_raymarch_depth: validates the views, sizes the {depth, omega} workspace, fills the
@@ -614,16 +646,24 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
         if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ctx->ev_h2d_done, 0);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D event");
     }
-    for (int k = 0; k < n_views; ++k) {
-        char* slot = base + (size_t)slots[k] * (2 * rgb + dep);
-        float* state = reinterpret_cast<float*>(slot + 2 * rgb);
-        float* dcur = reinterpret_cast<float*>(view_base + (size_t)k * dep);
-        if (rcur[k]) {
-            int rcode = ggt_refine_depth(ctx, W, H, rcur[k], rprev[k], 3, dcur, state, nullptr, nullptr, params, stream);
+    {   // all refined views in one batched call (two launches for the frame)
+        const uint8_t* bc[GGT_MAX_VIEWS]; const uint8_t* bp[GGT_MAX_VIEWS];
+        const float* bd[GGT_MAX_VIEWS]; float* bs[GGT_MAX_VIEWS];
+        int nb = 0;
+        for (int k = 0; k < n_views; ++k) {
+            char* slot = base + (size_t)slots[k] * (2 * rgb + dep);
+            float* state = reinterpret_cast<float*>(slot + 2 * rgb);
+            float* dcur = reinterpret_cast<float*>(view_base + (size_t)k * dep);
+            if (rcur[k]) {
+                bc[nb] = rcur[k]; bp[nb] = rprev[k]; bd[nb] = dcur; bs[nb] = state; ++nb;
+                dptr[k] = state;
+            } else {
+                dptr[k] = dcur;
+            }
+        }
+        if (nb > 0) {
+            int rcode = ggt_refine_depth_batch(ctx, nb, W, H, bc, bp, 3, bd, bs, nullptr, nullptr, params, stream);
             if (rcode != GGT_OK) return rcode;
-            dptr[k] = state;
-        } else {
-            dptr[k] = dcur;
         }
     }
     float* d_depth = reinterpret_cast<float*>(out_base);

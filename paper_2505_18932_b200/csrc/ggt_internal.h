@@ -63,6 +63,21 @@ struct GgtTemporalParams {
     GgtMaskView v[GGT_MAX_VIEWS];
 };
 
+struct GgtRefineView {
+    const uint8_t* rgb_cur;
+    const uint8_t* rgb_prev;
+    const float* depth_cur;
+    float* depth_state;
+    float* mask_out;       // optional
+    uint16_t* pooled_out;  // optional
+    uint16_t* cq;          // quarter-res block differences (context scratch)
+};
+
+struct GgtRefineViews {     // views of one ggt_refine_depth(_batch) call that have a previous colour image
+    int32_t n, pad_;
+    GgtRefineView v[GGT_MAX_VIEWS];
+};
+
 struct GgtFeatureView {
     float C[3];            // camera centre -R_k^T t_k
     float dist;            // |C_k - C_t|
@@ -141,10 +156,9 @@ struct ggt_volume {
 static inline int ggt_group_of(int dtype) { return dtype == GGT_F16 ? 4 : 2; }
 
 // ---- kernel launchers (each returns cudaError_t of the launch) ----------------------------------------
-cudaError_t ggt_launch_refine(int W, int H, const uint8_t* rgb_cur, const uint8_t* rgb_prev, int stride,
-                              const float* depth_cur, float* depth_state, float* mask_out,
-                              uint16_t* pooled_out, uint16_t* cq_scratch, float lambda_t, float beta,
-                              float theta, cudaStream_t st, int* n_launches);
+cudaError_t ggt_launch_refine(int W, int H, const GgtRefineViews& tab, int stride, float lambda_t, float beta, float theta,
+                              cudaStream_t st, int* n_launches);
+cudaError_t ggt_launch_first_frame(int W, int H, const float* depth_cur, float* depth_state, float* mask_out, cudaStream_t st);
 cudaError_t ggt_launch_weight_maps(const GgtWeightParams& p, cudaStream_t st);
 cudaError_t ggt_launch_integrate(const GgtIntegrateParams& p, int dtype, bool fused, cudaStream_t st);
 cudaError_t ggt_launch_temporal_weight(const GgtTemporalParams& p, cudaStream_t st);

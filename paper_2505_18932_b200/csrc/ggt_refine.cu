@@ -5,7 +5,8 @@
 // Readings P5-P8, P17 of DESIGN.md fix what the paper leaves open (L1 over RGB, 4x4 box sums, clipped
 // pooling window, half-pixel bilinear, valid-term handling).
 //
-// Two kernels per view:
+// Two kernels per call, for one view (ggt_refine_depth) or all views of a frame at once (ggt_refine_depth_batch,
+// blockIdx.z = view):
 //   k_block_diff   one thread per quarter-res cell: 4x4 box sums of both images, L1 over RGB  (integer)
 //   k_mask_blend   one CTA per 64x16 pixel tile: 3x3 max-pool + Eq. 1 on the 18x6 cells the tile's bilinear
 //                  footprint touches (shared memory), then per pixel bilinear x4 + Eq. 2, 128-bit accesses.
@@ -31,8 +32,10 @@ __device__ __forceinline__ void rgb4_sums(uint32_t w0, uint32_t w1, uint32_t w2,
 
 template <bool FAST>
 __global__ void __launch_bounds__(256)
-k_block_diff(int W, int H, int Wq, int Hq, const uint8_t* __restrict__ cur, const uint8_t* __restrict__ prev,
-             int stride, uint16_t* __restrict__ cq) {
+k_block_diff(int W, int H, int Wq, int Hq, const __grid_constant__ GgtRefineViews tab, int stride) {
+    const uint8_t* __restrict__ cur = tab.v[blockIdx.z].rgb_cur;
+    const uint8_t* __restrict__ prev = tab.v[blockIdx.z].rgb_prev;
+    uint16_t* __restrict__ cq = tab.v[blockIdx.z].cq;
     const int xq = blockIdx.x * 32 + threadIdx.x;
     const int yq = blockIdx.y * 8 + threadIdx.y;
     if (xq >= Wq || yq >= Hq) return;
@@ -68,9 +71,13 @@ k_block_diff(int W, int H, int Wq, int Hq, const uint8_t* __restrict__ cur, cons
 }
 
 __global__ void __launch_bounds__(256)
-k_mask_blend(int W, int H, int Wq, int Hq, const uint16_t* __restrict__ cq, const float* __restrict__ depth_cur,
-             float* __restrict__ depth_state, float* __restrict__ mask_out, uint16_t* __restrict__ pooled_out,
-             float lambda_t, float beta, float theta) {
+k_mask_blend(int W, int H, int Wq, int Hq, const __grid_constant__ GgtRefineViews tab, float lambda_t, float beta,
+             float theta) {
+    const uint16_t* __restrict__ cq = tab.v[blockIdx.z].cq;
+    const float* __restrict__ depth_cur = tab.v[blockIdx.z].depth_cur;
+    float* __restrict__ depth_state = tab.v[blockIdx.z].depth_state;
+    float* __restrict__ mask_out = tab.v[blockIdx.z].mask_out;
+    uint16_t* __restrict__ pooled_out = tab.v[blockIdx.z].pooled_out;
     __shared__ int s_cq[QH][QW];
     __shared__ float s_m[CH][CW];
     const int tid = threadIdx.x;
@@ -184,26 +191,25 @@ k_first_frame(size_t n, const float* __restrict__ depth_cur, float* __restrict__
 
 }  // namespace
 
-cudaError_t ggt_launch_refine(int W, int H, const uint8_t* rgb_cur, const uint8_t* rgb_prev, int stride,
-                              const float* depth_cur, float* depth_state, float* mask_out,
-                              uint16_t* pooled_out, uint16_t* cq_scratch, float lambda_t, float beta,
-                              float theta, cudaStream_t st, int* n_launches) {
-    if (!rgb_prev) {
-        const size_t n = (size_t)W * H;
-        k_first_frame<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, depth_cur, depth_state, mask_out);
-        *n_launches = 1;
-        return cudaGetLastError();
-    }
+// All views of `tab` have the same size and a previous colour image; one launch of each kernel, blockIdx.z = view.
+cudaError_t ggt_launch_refine(int W, int H, const GgtRefineViews& tab, int stride, float lambda_t, float beta, float theta,
+                              cudaStream_t st, int* n_launches) {
     const int Wq = (W + S - 1) / S, Hq = (H + S - 1) / S;
-    const dim3 blk(32, 8), grd((Wq + 31) / 32, (Hq + 7) / 8);
-    const bool fast = stride == 3 && (W % 4) == 0 && (((uintptr_t)rgb_cur | (uintptr_t)rgb_prev) & 3) == 0;
-    if (fast) k_block_diff<true><<<grd, blk, 0, st>>>(W, H, Wq, Hq, rgb_cur, rgb_prev, stride, cq_scratch);
-    else k_block_diff<false><<<grd, blk, 0, st>>>(W, H, Wq, Hq, rgb_cur, rgb_prev, stride, cq_scratch);
+    const dim3 blk(32, 8), grd((Wq + 31) / 32, (Hq + 7) / 8, tab.n);
+    bool fast = stride == 3 && (W % 4) == 0;
+    for (int k = 0; k < tab.n; ++k) fast = fast && (((uintptr_t)tab.v[k].rgb_cur | (uintptr_t)tab.v[k].rgb_prev) & 3) == 0;
+    if (fast) k_block_diff<true><<<grd, blk, 0, st>>>(W, H, Wq, Hq, tab, stride);
+    else k_block_diff<false><<<grd, blk, 0, st>>>(W, H, Wq, Hq, tab, stride);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    const dim3 grd2((W + TILE_W - 1) / TILE_W, (H + TILE_H - 1) / TILE_H);
-    k_mask_blend<<<grd2, 256, 0, st>>>(W, H, Wq, Hq, cq_scratch, depth_cur, depth_state, mask_out, pooled_out,
-                                       lambda_t, beta, theta);
+    const dim3 grd2((W + TILE_W - 1) / TILE_W, (H + TILE_H - 1) / TILE_H, tab.n);
+    k_mask_blend<<<grd2, 256, 0, st>>>(W, H, Wq, Hq, tab, lambda_t, beta, theta);
     *n_launches = 2;
+    return cudaGetLastError();
+}
+
+cudaError_t ggt_launch_first_frame(int W, int H, const float* depth_cur, float* depth_state, float* mask_out, cudaStream_t st) {
+    const size_t n = (size_t)W * H;
+    k_first_frame<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, depth_cur, depth_state, mask_out);
     return cudaGetLastError();
 }

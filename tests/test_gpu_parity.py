@@ -292,3 +292,35 @@ def test_frame_host_pipelined_without_host_sync():
     for f in range(F):
         ref = gp.frame(f)[0]
         assert torch.equal(outs[f][0], ref["depth"].cpu()) and torch.equal(outs[f][1], ref["conf"].cpu()), "frame %d" % f
+
+
+def test_refine_batch_equals_per_view_and_oracle():
+    """ggt_refine_depth_batch (all views of a frame in two launches) = the per-view call = the oracle, including a view
+    without history (first-frame rule) in the same batch."""
+    import torch
+    from paper_2505_18932_b200 import binding
+    H, W, V = 136, 200, 5
+    rng = np.random.default_rng(42)
+    ctx = binding.Context()
+    cur, prev, dep, st0 = [], [], [], []
+    for k in range(V):
+        p = rng.integers(0, 256, (H, W, 3), dtype=np.uint8)
+        c = np.clip(p.astype(np.int16) + rng.integers(-1, 2, p.shape), 0, 255).astype(np.uint8)
+        c[20 + 10 * k:60 + 10 * k, 30:90] = np.clip(c[20 + 10 * k:60 + 10 * k, 30:90].astype(np.int16) + 40 + 20 * k, 0, 255).astype(np.uint8)
+        cur.append(c); prev.append(p if k != 2 else None)                 # view 2 has no history
+        d = rng.uniform(0.5, 5, (H, W)).astype(np.float32); d[rng.uniform(size=(H, W)) < 0.05] = 0
+        s = rng.uniform(0.5, 5, (H, W)).astype(np.float32); s[rng.uniform(size=(H, W)) < 0.05] = 0
+        dep.append(d); st0.append(s)
+    theta = 8.0 / 255.0
+    g = lambda a: None if a is None else torch.from_numpy(a).cuda()
+    states = [g(s.copy()) for s in st0]
+    masks = [torch.empty((H, W), dtype=torch.float32, device="cuda") for _ in range(V)]
+    ctx.ggt_refine_depth_batch([g(c) for c in cur], [g(p) for p in prev], [g(d) for d in dep], states, mask_out=masks, theta=theta)
+    torch.cuda.synchronize()
+    for k in range(V):
+        if prev[k] is None:
+            o_out, o_M = dep[k], np.ones((H, W), np.float32)
+        else:
+            o_out, o_M, _, _ = oracle.refine(cur[k], prev[k], dep[k], st0[k], theta=theta)
+        assert np.array_equal(states[k].cpu().numpy().view(np.uint32), o_out.view(np.uint32)), k
+        assert np.array_equal(masks[k].cpu().numpy().view(np.uint32), o_M.view(np.uint32)), k
