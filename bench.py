@@ -432,6 +432,25 @@ def main():
             "ms_per_call": ms_r, "kernel_ms": k_ms, "evaluations_per_ray_mean": evals / n_t,
             "gsample_view_per_s": evals * inp.V / (k_ms / 1e3) / 1e9 if k_ms > 0 else None,
             "hit_fraction": float((dev.depth > 0).float().mean().item())}
+        # the paper's Table 4 shape for the same schedule: target and K = 4 views of 1352 x 1014
+        from paper_2505_18932_b200 import synth as _synth
+        rig_p = _synth.grid_rig(1352, 1014)
+        tgt_p = rig_p[5]
+        vi_p = _synth.nearest_views(tgt_p, rig_p, 4, exclude=5)
+        views_p = [rig_p[i] for i in vi_p]
+        dep_p = [torch.from_numpy(_synth.noisy_depth(_synth.raycast(c, wl.scene)[0], 1352, i, 0.01, 0.02)).cuda()
+                 for i, c in enumerate(views_p)]
+        n_p = 1352 * 1014
+        d_p, c_p = torch.empty(n_p, device="cuda"), torch.empty(n_p, device="cuda")
+        s_p = torch.zeros(n_p, dtype=torch.int32, device="cuda")
+        rmp_fn = lambda: dev.ctx.ggt_raymarch_depth(tgt_p, views_p, dep_p, zn, zf, depth=d_p, conf=c_p, steps=s_p)
+        ms_rp = timed(torch, None, rmp_fn, k, 3) / k
+        extra["paper_table4_shape"] = {
+            "call": "ggt_raymarch_depth, target and K = 4 views of 1352x1014 (the resolution of PAPER.md Table 4's 6 ms TSDF "
+                    "stage, GPU not stated), synthetic scene of this workload, weight maps included",
+            "ms_per_call": ms_rp, "evaluations_per_ray_mean": float(s_p.sum().item()) / n_p,
+            "hit_fraction": float((d_p > 0).float().mean().item())}
+        del dep_p, d_p, c_p, s_p
         # f-4: network-input geometry features of the guidance depth just produced
         feats = torch.empty((4 * inp.V, t.height, t.width), dtype=torch.float32, device="cuda")
         gdepth = dev.depth.clone()
