@@ -31,6 +31,7 @@ def test_struct_sizes_match_header():
     assert ctypes.sizeof(binding.ggt_camera) == 4 * 4 + 9 * 4 + 3 * 4 + 2 * 4
     assert ctypes.sizeof(binding.ggt_refine_params) == 20
     assert ctypes.sizeof(binding.ggt_volume_desc) == 56
+    assert ctypes.sizeof(binding.ggt_raymarch_params) == 40
 
 
 def test_volume_bytes_layout():

@@ -29,7 +29,7 @@ def guidance_depth(wl, tgt, rng, holes=0.03):
     return d
 
 
-@pytest.mark.parametrize("name,scale", [("C1", 1.0), ("C2", 1.0), ("C3", 0.5), ("C4", 0.25), ("C5", 0.25)])
+@pytest.mark.parametrize("name,scale", [("C1", 1.0), ("C2", 1.0), ("C3", 1.0), ("C4", 0.5), ("C5", 0.5)])
 def test_features_configs(name, scale):
     wl = synth.workload(name, scale=scale)
     tgt = wl.targets(0)[0]
