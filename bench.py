@@ -144,7 +144,7 @@ class DeviceRun:
         self.torch, self.b, self.inp, self.fused = torch, binding, inp, fused
         wl = inp.wl
         self.ctx = binding.Context()
-        self.ctx.ggt_set_workspace(inp.V + 1, max(inp.W, inp.target.width), max(inp.H, inp.target.height))   # + the previous output depth (Eq. 3 leg)
+        self.ctx.ggt_set_workspace(max(inp.V + 1, len(inp.view_ids)), max(inp.W, inp.target.width), max(inp.H, inp.target.height))   # + the previous output depth (Eq. 3 leg)
         self.vols = []
         for t in inp.targets:
             vol = self.ctx.ggt_volume_bind(t.width, t.height, wl.z_bins,
@@ -157,7 +157,9 @@ class DeviceRun:
             self.depth_by = [{v: torch.from_numpy(np.array(d[v][0])).cuda() for v in inp.view_ids} for d in inp.data_by_view]
             self.rgb_by = [{v: torch.from_numpy(np.array(d[v][1])).cuda() for v in inp.view_ids} for d in inp.data_by_view]
             self.state_by = {v: self.depth_by[0][v].clone() for v in inp.view_ids}
-            self.tviews = [[wl.rig[v] for v in vi] for vi in inp.vis]
+            pos = {v: i for i, v in enumerate(inp.view_ids)}
+            self.rig_views = [wl.rig[v] for v in inp.view_ids]
+            self.view_index = [[pos[v] for v in vi] for vi in inp.vis]
         self.depth_in = [[torch.from_numpy(np.array(d)).cuda() for d, _ in fr] for fr in inp.data]
         self.rgb_in = [[torch.from_numpy(np.array(r)).cuda() if r is not None else None for _, r in fr] for fr in inp.data]
         self.state = [self.depth_in[0][k].clone() for k in range(inp.V)]
@@ -176,9 +178,10 @@ class DeviceRun:
             ids = inp.view_ids
             ctx.ggt_refine_depth_batch([self.rgb_by[cur][v] for v in ids], [self.rgb_by[prev][v] for v in ids],
                                        [self.depth_by[cur][v] for v in ids], [self.state_by[v] for v in ids], **REFINE)
-            for ti, t in enumerate(inp.targets):
-                depths = [self.state_by[v] for v in inp.vis[ti]]
-                ctx.ggt_integrate(self.vols[ti], t, self.tviews[ti], depths, self.flags)
+            # the 8 targets of the frame in one batched call: the weight maps of the rig views are computed once
+            ctx.ggt_integrate_batch(self.vols, inp.targets, self.rig_views, [self.state_by[v] for v in ids], self.view_index,
+                                    self.flags)
+            for ti in range(len(inp.targets)):
                 ctx.ggt_extract_depth(self.vols[ti], self.depth, self.conf)
             return
         if inp.wl.colour:

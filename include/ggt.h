@@ -160,6 +160,17 @@ int ggt_refine_depth_batch(ggt_ctx* ctx, int32_t n_views, int32_t width, int32_t
 int ggt_integrate(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
                   const ggt_camera* views, const float* const* dev_depths, uint32_t flags, void* stream);
 
+/* Batched novel views (BASELINE.json:configs[4]): n_targets targets of one frame, each with its own volume and
+ * its own n_views input views chosen from the n_rig_views views of the frame.  The {depth, omega} maps (Eq. 11-12)
+ * of the rig views are computed ONCE and shared by the targets; otherwise exactly n_targets ggt_integrate calls.
+ *   vols, targets     HOST arrays of n_targets volume handles / cameras (targets[t] matches vols[t]; the volumes
+ *                     share w_sigma0 / w_clip / w_window)
+ *   rig_views, dev_depths  HOST arrays of n_rig_views cameras / DEVICE depth pointers, 1 <= n_rig_views <= GGT_MAX_VIEWS
+ *   view_index        HOST, n_targets x n_views indices into rig_views (row t = the views of target t, in fusion order) */
+int ggt_integrate_batch(ggt_ctx* ctx, int32_t n_targets, ggt_volume* const* vols, const ggt_camera* targets,
+                        int32_t n_rig_views, const ggt_camera* rig_views, const float* const* dev_depths,
+                        int32_t n_views, const int32_t* view_index, uint32_t flags, void* stream);
+
 /* ---- step a7: zero-crossing depth (reading P13) ------------------------------------- */
 /* Outputs are fp32 / int32 H_t x W_t; any may be NULL.  Miss: depth 0, conf 0, bin -1. */
 int ggt_extract_depth(ggt_ctx* ctx, const ggt_volume* vol, float* dev_depth, float* dev_conf,

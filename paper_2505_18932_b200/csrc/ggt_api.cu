@@ -339,11 +339,11 @@ int ggt_refine_depth(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t*
                                   &dev_depth_state, &dev_mask_out, &dev_pooled_out, params, stream);
 }
 
-// Shared by ggt_integrate and ggt_raymarch_depth: validates the views, sizes the {depth, omega} workspace, fills the
-// per-view kernel parameters (relative transform a4, map pointers) and launches the weight-map pre-pass (a3).
-static int prepare_views(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views, const ggt_camera* views,
-                         const float* const* dev_depths, const float* const* dev_weights, float w_sigma0, float w_clip, int32_t w_window,
-                         GgtViewParams* vp, cudaStream_t st) {
+// a3: validates the views, sizes the {depth, omega} workspace and launches the weight-map pre-pass for all of them
+// (one launch); map_out[k] is the device address of view k's zero-padded {depth, omega} map.
+static int prepare_maps(ggt_ctx* ctx, int32_t n_views, const ggt_camera* views, const float* const* dev_depths,
+                        const float* const* dev_weights, float w_sigma0, float w_clip, int32_t w_window,
+                        const float2** map_out, cudaStream_t st) {
     size_t need = 0;
     for (int k = 0; k < n_views; ++k) {
         if (views[k].width <= 0 || views[k].height <= 0 || views[k].width > 32767 || views[k].height > 32767)
@@ -366,14 +366,7 @@ static int prepare_views(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views
     wp.n_views = n_views; wp.window = w_window;
     wp.sigma0 = w_sigma0; wp.c2 = w_clip * w_clip;
     for (int k = 0; k < n_views; ++k) {
-        float hm[9], ev[3];
-        relative_transform(*target, views[k], hm, ev);
-        for (int i = 0; i < 6; ++i) vp[k].nh[i] = -hm[i];
-        for (int i = 0; i < 3; ++i) vp[k].h2[i] = hm[6 + i];
-        vp[k].ne[0] = -ev[0]; vp[k].ne[1] = -ev[1]; vp[k].e2 = ev[2];
-        vp[k].map = reinterpret_cast<const float2*>(w);
-        vp[k].width = views[k].width; vp[k].height = views[k].height;
-        vp[k].stride = (uint32_t)views[k].width + 1u;
+        map_out[k] = reinterpret_cast<const float2*>(w);
         wp.v[k].depth = dev_depths[k]; wp.v[k].out = reinterpret_cast<float2*>(w);
         wp.v[k].weight = dev_weights ? dev_weights[k] : nullptr;
         wp.v[k].width = views[k].width; wp.v[k].height = views[k].height;
@@ -388,6 +381,40 @@ static int prepare_views(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views
         ctx->inputs_free_pending = true;
     }
     return GGT_OK;
+}
+
+// a4: the relative transform target -> view (12 floats) and the view's map for the kernels
+static void fill_view_params(const ggt_camera& target, const ggt_camera& view, const float2* map, GgtViewParams& vp) {
+    float hm[9], ev[3];
+    relative_transform(target, view, hm, ev);
+    for (int i = 0; i < 6; ++i) vp.nh[i] = -hm[i];
+    for (int i = 0; i < 3; ++i) vp.h2[i] = hm[6 + i];
+    vp.ne[0] = -ev[0]; vp.ne[1] = -ev[1]; vp.e2 = ev[2];
+    vp.map = map;
+    vp.width = view.width; vp.height = view.height;
+    vp.stride = (uint32_t)view.width + 1u;
+}
+
+// Shared by ggt_integrate and ggt_raymarch_depth: a3 + a4 for one target.
+static int prepare_views(ggt_ctx* ctx, const ggt_camera* target, int32_t n_views, const ggt_camera* views,
+                         const float* const* dev_depths, const float* const* dev_weights, float w_sigma0, float w_clip, int32_t w_window,
+                         GgtViewParams* vp, cudaStream_t st) {
+    const float2* maps[GGT_MAX_VIEWS];
+    const int rc = prepare_maps(ctx, n_views, views, dev_depths, dev_weights, w_sigma0, w_clip, w_window, maps, st);
+    if (rc != GGT_OK) return rc;
+    for (int k = 0; k < n_views; ++k) fill_view_params(*target, views[k], maps[k], vp[k]);
+    return GGT_OK;
+}
+
+// same-size / shared-w detection for the integrate kernel's fast marches
+static void detect_fast_paths(GgtIntegrateParams& p, int32_t n_views) {
+    p.same_size = 1;
+    for (int k = 1; k < n_views; ++k)
+        if (p.v[k].width != p.v[0].width || p.v[k].height != p.v[0].height) p.same_size = 0;
+    // parallel rig: w_k(z) = fma(z, fma(h20, uc, fma(h21, vc, h22)), e2) has the same bits in every view
+    p.shared_w = p.same_size && n_views >= 2;
+    for (int k = 1; k < n_views; ++k)
+        if (memcmp(p.v[k].h2, p.v[0].h2, sizeof p.v[0].h2) != 0 || memcmp(&p.v[k].e2, &p.v[0].e2, sizeof(float)) != 0) p.shared_w = 0;
 }
 
 // Shared front end of ggt_integrate / ggt_integrate_extract: validation, workspace, weight maps, launch.
@@ -419,13 +446,7 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
         if (rc != GGT_OK) return rc;
     }
     StageTimer tm(ctx, GGT_STAGE_INTEGRATE, st);
-    p.same_size = 1;
-    for (int k = 1; k < n_views; ++k)
-        if (views[k].width != views[0].width || views[k].height != views[0].height) p.same_size = 0;
-    // parallel rig: w_k(z) = fma(z, fma(h20, uc, fma(h21, vc, h22)), e2) has the same bits in every view
-    p.shared_w = p.same_size && n_views >= 2;
-    for (int k = 1; k < n_views; ++k)
-        if (memcmp(p.v[k].h2, p.v[0].h2, sizeof p.v[0].h2) != 0 || memcmp(&p.v[k].e2, &p.v[0].e2, sizeof(float)) != 0) p.shared_w = 0;
+    detect_fast_paths(p, n_views);
     cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, fused, st);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "integrate launch");
     ctx->launches += 1;
@@ -447,6 +468,56 @@ int ggt_integrate_extract(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
                           const ggt_camera* views, const float* const* dev_depths, uint32_t flags,
                           float* dev_depth, float* dev_conf, int32_t* dev_bin, void* stream) {
     return integrate_impl(ctx, vol, target, n_views, views, dev_depths, nullptr, flags, true, dev_depth, dev_conf, dev_bin, stream);
+}
+
+int ggt_integrate_batch(ggt_ctx* ctx, int32_t n_targets, ggt_volume* const* vols, const ggt_camera* targets,
+                        int32_t n_rig_views, const ggt_camera* rig_views, const float* const* dev_depths,
+                        int32_t n_views, const int32_t* view_index, uint32_t flags, void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    if (!vols || !targets || !rig_views || !dev_depths || !view_index) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL argument to ggt_integrate_batch");
+    if (n_targets < 1) return fail(ctx, GGT_ERR_SHAPE, "n_targets %d", n_targets);
+    if (n_rig_views < 1 || n_rig_views > GGT_MAX_VIEWS) return fail(ctx, GGT_ERR_SHAPE, "n_rig_views %d not in [1, %d]", n_rig_views, GGT_MAX_VIEWS);
+    if (n_views < 1 || n_views > n_rig_views) return fail(ctx, GGT_ERR_SHAPE, "n_views %d not in [1, n_rig_views]", n_views);
+    if (flags != GGT_OVERWRITE && flags != GGT_ACCUMULATE) return fail(ctx, GGT_ERR_INVALID_ARG, "flags %u", flags);
+    for (int t = 0; t < n_targets; ++t) {
+        if (!vols[t]) return fail(ctx, GGT_ERR_INVALID_ARG, "vols[%d] is NULL", t);
+        if (targets[t].width != vols[t]->desc.width || targets[t].height != vols[t]->desc.height)
+            return fail(ctx, GGT_ERR_SHAPE, "target %d does not match its volume", t);
+        if (!(targets[t].fx > 0.0f) || !(targets[t].fy > 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "target %d focal length", t);
+        if (vols[t]->desc.w_sigma0 != vols[0]->desc.w_sigma0 || vols[t]->desc.w_clip != vols[0]->desc.w_clip ||
+            vols[t]->desc.w_window != vols[0]->desc.w_window)
+            return fail(ctx, GGT_ERR_INVALID_ARG, "the volumes of one batch must share the Eq. 11-12 parameters");
+        for (int k = 0; k < n_views; ++k) {
+            const int idx = view_index[t * n_views + k];
+            if (idx < 0 || idx >= n_rig_views) return fail(ctx, GGT_ERR_INVALID_ARG, "view_index[%d][%d] = %d", t, k, idx);
+        }
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const float2* maps[GGT_MAX_VIEWS];
+    int rc = prepare_maps(ctx, n_rig_views, rig_views, dev_depths, nullptr, vols[0]->desc.w_sigma0, vols[0]->desc.w_clip,
+                          vols[0]->desc.w_window, maps, st);                      // the weight maps, once per frame
+    if (rc != GGT_OK) return rc;
+    for (int t = 0; t < n_targets; ++t) {
+        const ggt_volume* vol = vols[t];
+        GgtIntegrateParams p;
+        memset(&p, 0, sizeof p);
+        p.Wt = vol->desc.width; p.Ht = vol->desc.height; p.D = vol->desc.bins;
+        p.n_views = n_views; p.n_groups = vol->n_groups;
+        p.plane = (unsigned long long)vol->desc.width * (unsigned long long)vol->desc.height;
+        p.accumulate = flags == GGT_ACCUMULATE ? 1 : 0;
+        p.decay = vol->desc.decay; p.cap = vol->desc.weight_cap;
+        p.tables = vol->dev_tables; p.voxels = vol->dev_voxels;
+        for (int k = 0; k < n_views; ++k) {
+            const int idx = view_index[t * n_views + k];
+            fill_view_params(targets[t], rig_views[idx], maps[idx], p.v[k]);
+        }
+        detect_fast_paths(p, n_views);
+        StageTimer tm(ctx, GGT_STAGE_INTEGRATE, st);
+        cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, false, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "integrate launch");
+        ctx->launches += 1;
+    }
+    return GGT_OK;
 }
 
 int ggt_extract_depth(ggt_ctx* ctx, const ggt_volume* vol, float* dev_depth, float* dev_conf, int32_t* dev_bin,

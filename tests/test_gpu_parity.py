@@ -324,3 +324,35 @@ def test_refine_batch_equals_per_view_and_oracle():
             o_out, o_M, _, _ = oracle.refine(cur[k], prev[k], dep[k], st0[k], theta=theta)
         assert np.array_equal(states[k].cpu().numpy().view(np.uint32), o_out.view(np.uint32)), k
         assert np.array_equal(masks[k].cpu().numpy().view(np.uint32), o_M.view(np.uint32)), k
+
+
+def test_integrate_batch_equals_per_target_calls():
+    """ggt_integrate_batch (8 targets of a C5-shaped frame, weight maps computed once) leaves every volume exactly as
+    per-target ggt_integrate calls do, over two accumulated frames."""
+    import torch
+    from paper_2505_18932_b200 import binding
+    wl = synth.workload("C5", scale=0.125)
+    ctx_a, ctx_b = binding.Context(), binding.Context()
+    targets = wl.targets(0)
+    vis = [wl.views_for(t) for t in targets]
+    ids = sorted(set(v for vi in vis for v in vi))
+    pos = {v: i for i, v in enumerate(ids)}
+    rig_views = [wl.rig[v] for v in ids]
+    mk = lambda c: [c.ggt_volume_bind(t.width, t.height, wl.z_bins, weight_cap=wl.weight_cap) for t in targets]
+    va, vb = mk(ctx_a), mk(ctx_b)
+    for v in va + vb:
+        v.ggt_volume_reset()
+    for f in range(2):
+        dep = {v: torch.from_numpy(wl.view_inputs(f, v)[0]).cuda() for v in ids}
+        ctx_a.ggt_integrate_batch(va, targets, rig_views, [dep[v] for v in ids], [[pos[v] for v in vi] for vi in vis],
+                                  binding.GGT_ACCUMULATE)
+        for t, vi, vol in zip(targets, vis, vb):
+            ctx_b.ggt_integrate(vol, t, [wl.rig[v] for v in vi], [dep[v] for v in vi], binding.GGT_ACCUMULATE)
+    torch.cuda.synchronize()
+    for a, b in zip(va, vb):
+        Ta, Wa = a.ggt_volume_export()
+        Tb, Wb = b.ggt_volume_export()
+        assert torch.equal(Ta, Tb) and torch.equal(Wa, Wb)
+    assert float((Wa > 0).float().mean()) > 0.1
+    with pytest.raises(binding.GgtError):
+        ctx_a.ggt_integrate_batch(va, targets, rig_views, [dep[v] for v in ids], [[99] * len(vis[0])] * len(targets))
