@@ -142,7 +142,7 @@ def test_fused_persistent_fp16_matches():
 
 
 # ---- edge cases ------------------------------------------------------------------------------------------
-def _simple(n_views, D, dtype_name, W=70, H=37, invalid=False, seed=11, accumulate=False, frames=1):
+def _simple(n_views, D, dtype_name, W=70, H=37, invalid=False, seed=11, accumulate=False, frames=1, fused=False):
     """Random rig around the origin, arbitrary (ragged) sizes and view counts."""
     import torch
     from paper_2505_18932_b200 import binding
@@ -169,12 +169,16 @@ def _simple(n_views, D, dtype_name, W=70, H=37, invalid=False, seed=11, accumula
                                  accumulate=accumulate, half_storage=dtype_name == "f16")
         od, oc, ob = oracle.extract(z, T, Wt)
         gd = [torch.from_numpy(d).cuda() for d in depths]
-        ctx.ggt_integrate(vol, tgt, views, gd, binding.GGT_ACCUMULATE if accumulate else binding.GGT_OVERWRITE)
         n = W * H
         depth = torch.empty(n, dtype=torch.float32, device="cuda")
         conf = torch.empty(n, dtype=torch.float32, device="cuda")
         bins = torch.empty(n, dtype=torch.int32, device="cuda")
-        ctx.ggt_extract_depth(vol, depth, conf, bins)
+        flags = binding.GGT_ACCUMULATE if accumulate else binding.GGT_OVERWRITE
+        if fused:
+            ctx.ggt_integrate_extract(vol, tgt, views, gd, flags, depth, conf, bins)
+        else:
+            ctx.ggt_integrate(vol, tgt, views, gd, flags)
+            ctx.ggt_extract_depth(vol, depth, conf, bins)
         o = dict(rays=None, T=T, W=Wt, depth=od, conf=oc, bins=ob)
         g = dict(vol=vol, depth=depth, conf=conf, bins=bins)
         st = helpers.compare_frame(o, g, z, tau)
@@ -186,6 +190,13 @@ def _simple(n_views, D, dtype_name, W=70, H=37, invalid=False, seed=11, accumula
 def test_view_counts(n_views):
     st, _ = _simple(n_views, 24, "f32")
     assert st["T_bitexact"]
+
+
+@pytest.mark.parametrize("n_views", [3, 5, 6, 7, 9, 12])
+@pytest.mark.parametrize("dtype_name,accumulate,fused", [("f16", True, False), ("f32", True, True), ("f16", False, True)])
+def test_view_counts_all_kernel_variants(n_views, dtype_name, accumulate, fused):
+    """odd view counts run the pipelined march with a ragged last unit: every storage / mode / fused variant"""
+    _simple(n_views, 22, dtype_name, accumulate=accumulate, frames=2 if accumulate else 1, fused=fused)
 
 
 @pytest.mark.parametrize("D,dtype_name", [(2, "f32"), (3, "f32"), (33, "f32"), (5, "f16"), (33, "f16"), (130, "f16")])
