@@ -388,7 +388,15 @@ def main():
     traffic_file = os.path.join(ROOT, "profiles", "traffic_integrate.json")
     if os.path.exists(traffic_file):
         with open(traffic_file) as fh:
-            roofline["traffic"] = json.load(fh).get(wl.name + ("_fused" if args.fused else ""))
+            tj = json.load(fh)
+        roofline["traffic"] = tj.get(wl.name + ("_fused" if args.fused else ""))
+        wi = tj.get(wl.name + "_warp_instructions")
+        if wi and not args.fused and integ_ms > 0:
+            # the kernel's practical limit: one warp instruction per SM sub-partition per clock (148 SMs x 4 x 1.965 GHz);
+            # the instruction count is the ncu-measured one of the committed profile (static for this workload)
+            peak_issue = 148 * 4 * 1.965e9
+            roofline["issue"] = {"warp_instructions_per_launch": wi, "peak_warp_instructions_per_s": peak_issue,
+                                 "frac": wi / peak_issue / (integ_ms / 1e3)}
 
     # ---- e2e: host buffers through ggt_frame_host, result needed on the host every step ----------------
     if inp.multi:

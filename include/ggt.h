@@ -100,10 +100,11 @@ int64_t ggt_launch_count(const ggt_ctx* ctx);
 int ggt_profile_enable(ggt_ctx* ctx, int32_t enable);
 int ggt_profile_collect(ggt_ctx* ctx, double* host_ms, int64_t* host_count);
 
-/* Test hook (determinism contract, P14): the integrate kernel forms 1/w and A/W with its own
- * branch-free packed sequences; this runs them on n pairs (dev_a[i], dev_b[i]), b > 0, and ADDS to
- * dev_mismatch[0] / [1] the number of elements whose reciprocal 1/b / quotient a/b differ in any bit from the
- * IEEE-754 round-to-nearest results (__frcp_rn, __fdiv_rn).  n even; dev_mismatch zeroed by the caller. */
+/* Test hook (determinism contract, P14): the kernels form 1/w, A/W, sqrt and x/49 with their own
+ * branch-free sequences; this runs them on n pairs (dev_a[i], dev_b[i]), b > 0, and ADDS to dev_mismatch[0..3] the
+ * number of elements whose reciprocal 1/b, quotient a/b (packed and scalar forms), square root sqrt(b) and quotient
+ * b/49 differ in any bit from the IEEE-754 round-to-nearest results (__frcp_rn, __fdiv_rn, __fsqrt_rn).  n even;
+ * dev_mismatch: 4 words zeroed by the caller. */
 int ggt_selftest_arith(ggt_ctx* ctx, int64_t n, const float* dev_a, const float* dev_b, uint32_t* dev_mismatch,
                        void* stream);
 

@@ -187,13 +187,13 @@ class Context:
         return {k: (ms[i], int(n[i])) for i, k in enumerate(("refine", "weight", "integrate", "extract", "raymarch"))}
 
     def ggt_selftest_arith(self, a, b):
-        """(reciprocal mismatches, division mismatches) of the kernel's arithmetic vs IEEE on cuda tensors a, b."""
+        """(reciprocal, division, sqrt, x/49) mismatch counts of the kernels' arithmetic vs IEEE on cuda tensors a, b."""
         import torch
-        out = torch.zeros(2, dtype=torch.int32, device="cuda")
+        out = torch.zeros(4, dtype=torch.int32, device="cuda")
         self.check(self.lib.ggt_selftest_arith(self.h, a.numel(), a.data_ptr(), b.data_ptr(), out.data_ptr(), _stream()),
                    "ggt_selftest_arith")
         r = out.cpu().numpy()
-        return int(r[0]), int(r[1])
+        return int(r[0]), int(r[1]), int(r[2]), int(r[3])
 
     def ggt_set_workspace(self, n_views: int, width: int, height: int):
         import torch

@@ -365,6 +365,7 @@ static int prepare_maps(ggt_ctx* ctx, int32_t n_views, const ggt_camera* views, 
     memset(&wp, 0, sizeof wp);
     wp.n_views = n_views; wp.window = w_window;
     wp.sigma0 = w_sigma0; wp.c2 = w_clip * w_clip;
+    wp.fast_ok = (w_sigma0 >= 1e-20f && w_sigma0 <= 1e20f) ? 1 : 0;
     for (int k = 0; k < n_views; ++k) {
         map_out[k] = reinterpret_cast<const float2*>(w);
         wp.v[k].depth = dev_depths[k]; wp.v[k].out = reinterpret_cast<float2*>(w);

@@ -103,6 +103,8 @@ struct GgtWeightView {
 struct GgtWeightParams {    // all views of one ggt_integrate call: one launch, blockIdx.z = view
     int32_t n_views, window;
     float sigma0, c2;      // c2 = clip * clip (one fp32 multiply, as the oracle states it)
+    int32_t fast_ok;       // sigma0 within [1e-20, 1e20]: the branch-free division / sqrt fast paths are exact
+    int32_t pad_;
     GgtWeightView v[GGT_MAX_VIEWS];
 };
 

@@ -20,22 +20,6 @@
 
 namespace {
 
-// -1/w (IEEE for normal w) of one lane: the scalar form of neg_rcp2
-__device__ __forceinline__ float neg_rcp1(float w) {
-    const float n0 = rcp_neg_approx(w);
-    const float e = fmaf(w, n0, 1.0f);
-    return fmaf(n0, e, n0);
-}
-
-// a / b given na = -a: the scalar form of div2_neg (fast path of IEEE division; exact for normal b > 0 and a normal
-// or zero quotient, which holds for sums of omega in [0.05, 16] and |A| <= tau * W)
-__device__ __forceinline__ float div1_neg(float na, float b) {
-    const float nr = neg_rcp1(b);
-    const float q = fmaf(na, nr, 0.0f);
-    const float nrem = fmaf(b, q, na);
-    return fmaf(nr, nrem, q);
-}
-
 struct RayView {            // per-ray, per-view constants: -(H_k rows 0, 1 . (uc, vc, 1)) and H_k row 2 . (uc, vc, 1)
     float nbx, nby, bw;
 };

@@ -28,12 +28,21 @@ constexpr int SW = 32 + 2 * R, SH = BH + 2 * R;   // 38 pairs x 22 rows
 
 __device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 
-__device__ __forceinline__ float omega_of(float D0, float nu, float sigma0, int window) {
+// Eq. 11: omega = min(sigma0 / sqrt(nu / 49), 1).  The three IEEE operations run as their branch-free fast paths
+// (ggt_packed.cuh; verified bit for bit against __fdiv_rn / __fsqrt_rn by ggt_selftest_arith) wherever all operands and
+// results are normal numbers far from the exponent limits -- every realistic depth map -- and as the compiler's
+// intrinsics otherwise.
+__device__ __forceinline__ float omega_of(float D0, float nu, float sigma0, int window, bool fast_ok) {
     if (!(D0 > 0.0f)) return 0.0f;
     if (window == 0 || nu == 0.0f) return 1.0f;
-    const float v = __fdiv_rn(nu, 49.0f);
-    const float sd = __fsqrt_rn(v);
-    const float w = __fdiv_rn(sigma0, sd);
+    float w;
+    if (fast_ok && nu >= 1e-30f && nu <= 1e30f) {
+        w = div1_neg(-sigma0, sqrt1(div49(nu)));
+    } else {
+        const float v = __fdiv_rn(nu, 49.0f);
+        const float sd = __fsqrt_rn(v);
+        w = __fdiv_rn(sigma0, sd);
+    }
     return w < 1.0f ? w : 1.0f;
 }
 
@@ -116,7 +125,7 @@ k_weight_map(const GgtWeightParams p) {
             if (xs[l] > W) continue;
             // the zero row / column the clamped gathers land on, and invalid pixels: {0, 0}
             const bool z = y == H || xs[l] == W || !(D[l] > 0.0f);
-            out[row + xs[l]] = z ? make_float2(0.0f, 0.0f) : make_float2(D[l], omega_of(D[l], nu[l], p.sigma0, p.window));
+            out[row + xs[l]] = z ? make_float2(0.0f, 0.0f) : make_float2(D[l], omega_of(D[l], nu[l], p.sigma0, p.window, p.fast_ok != 0));
         }
     }
 }

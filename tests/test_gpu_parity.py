@@ -47,14 +47,18 @@ def test_fast_reciprocal_and_division():
         # numerators: |a| <= 16 * b-ish magnitudes as in a weighted mean, random sign, plus exact zeros
         a = (torch.rand(b.shape, generator=g, device="cuda") * 2 - 1) * b * 0.3
         a[::97] = 0.0
-        r, q = ctx.ggt_selftest_arith(a, b)
-        assert r == 0 and q == 0, (start, r, q)
+        r, q, sq, c49 = ctx.ggt_selftest_arith(a, b)
+        assert r == 0 and q == 0 and sq == 0 and c49 == 0, (start, r, q, sq, c49)
         total += b.numel()
     assert total > 3e8
     # weights and numerators in the ranges the TSDF tail sees: Wn in [0.05, 16], |A| <= tau * Wn
     b = torch.rand(1 << 24, generator=g, device="cuda") * 16 + 0.05
     a = (torch.rand(1 << 24, generator=g, device="cuda") * 2 - 1) * b * 0.25
-    assert ctx.ggt_selftest_arith(a, b) == (0, 0)
+    assert ctx.ggt_selftest_arith(a, b) == (0, 0, 0, 0)
+    # the ranges Eq. 11-12 sees: nu in [1e-16, 49 * clip^2], nu / 49, its square root
+    b = torch.exp(torch.rand(1 << 24, generator=g, device="cuda") * 34.0 - 37.0)            # 1e-16 .. 0.05
+    a = torch.full_like(b, 0.001)
+    assert ctx.ggt_selftest_arith(a, b) == (0, 0, 0, 0)
 
 
 # ---- refine (a1-a2) ---------------------------------------------------------------------------------
