@@ -741,10 +741,11 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
     float* d_depth = reinterpret_cast<float*>(out_base);
     float* d_conf = reinterpret_cast<float*>(out_base + out);
     ctx->record_inputs_free = true;
-    int rcode = ggt_integrate(ctx, vol, target, n_views, views, dptr, flags, stream);
+    // a3-a7 in one pass: the result the host wants comes out of the integrate kernel itself (same bits as
+    // ggt_integrate followed by ggt_extract_depth, without re-reading the volume)
+    int rcode = ggt_integrate_extract(ctx, vol, target, n_views, views, dptr, flags, host_depth ? d_depth : nullptr,
+                                      host_conf ? d_conf : nullptr, nullptr, stream);
     ctx->record_inputs_free = false;
-    if (rcode != GGT_OK) return rcode;
-    rcode = ggt_extract_depth(ctx, vol, host_depth ? d_depth : nullptr, host_conf ? d_conf : nullptr, nullptr, stream);
     if (rcode != GGT_OK) return rcode;
     const size_t ob = (size_t)vol->desc.width * vol->desc.height * 4;
     if (host_depth) {
