@@ -279,10 +279,10 @@ def oracle_step(inp, ray_every, cur=1):
                   "rays": int(rays.size), "measured_s": t3 - t0}
 
 
-def cpu_baseline(inp, ray_every=8):
+def cpu_baseline(inp, ray_every=2):
     full, parts = oracle_step(inp, ray_every)
     return {"value": inp.vv_per_step / full / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": "one %s step: refine + weight maps of all %d views in full, integrate + extract on every %dth "
+            "sample": "one %s step: refine + weight maps of all %d views in full, integrate + extract on every %d-th "
                       "target ray (%d rays), ray part scaled by the sampling ratio; %.1f s of CPU work, "
                       "extrapolated %.1f s per frame; host has %d cores, the oracle is single-threaded"
                       % (inp.wl.name, inp.V, ray_every, parts["rays"], parts["measured_s"], full, os.cpu_count() or 0),
