@@ -41,7 +41,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         def compile_unit(i):
             src, defs = UNITS[i]
             obj = os.path.join(tmpdir, "u%d.o" % i)
-            cmd = [nvcc] + NVCC_FLAGS + defs + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, os.path.join(CSRC, src)]
+            cmd = [nvcc] + NVCC_FLAGS + defs + os.environ.get("GGT_EXTRA_NVCC_FLAGS", "").split() + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, os.path.join(CSRC, src)]
             r = subprocess.run(cmd, capture_output=True, text=True)
             if verbose or r.returncode != 0:
                 sys.stderr.write(r.stdout + r.stderr)
