@@ -34,10 +34,15 @@
 // T3 view-order invariance, T4 brute-force fp64 per-voxel, T5 Eq. 1 closed forms, T6 Eq. 2 EMA,
 // T7 Eq. 11-12 closed forms (0.050518), T8 cut/clamp sweep, T9 running-average closed form, T10 extract,
 // T11-T14 raymarch (planes / sphere closed form, dense fp64 first-crossing brute force, coincident camera,
-// closed-form evaluation counts).
+// closed-form evaluation counts), T15-T18 temporal weight (Eq. 13 closed forms, fp64 brute-force mask gather,
+// Eq. 14 recursion in closed form, variance reduction), T19-T22 network-input features (plane / sphere normals,
+// fp64 ray dot products and constant maps, undefined pixels).
 // Parity unpinned (choices, not derivable): the VALUES of tau in C2-C5 (P3), the
 // dead-zone threshold semantics (P6), decay/cap without mask gate (P9-P10), the border rule of
-// Eq. 12 (P11), the confidence output (P13).
+// Eq. 12 (P11), the confidence output (P13); in orc_raymarch the min_step / max_evals / unobserved-sample
+// rules and the confidence (M2-M4, M6); in orc_temporal_weight the gather that stands in for the paper's
+// forward splat of the masks, without an occlusion test (F1); in orc_features the finite-difference stencil
+// of the normal (G2).
 #include <cmath>
 #include <cstdint>
 #include <cstring>
