@@ -623,6 +623,7 @@ int ggt_guidance_features(ggt_ctx* ctx, const ggt_camera* target, const float* d
     memset(&p, 0, sizeof p);
     p.W = target->width; p.H = target->height; p.n_views = n_views;
     p.fx = target->fx; p.fy = target->fy; p.cx = target->cx; p.cy = target->cy;
+    p.fast_ok = (target->fx >= 1e-10f && target->fx <= 1e10f && target->fy >= 1e-10f && target->fy <= 1e10f) ? 1 : 0;
     for (int i = 0; i < 9; ++i) p.R[i] = target->R[i];
     for (int i = 0; i < 3; ++i) p.t[i] = target->t[i];
     camera_centre(*target, p.Ct);

@@ -6,8 +6,10 @@
 // without a neighbour in either axis), oriented towards the camera; rays = unit vectors from the camera centres to the
 // surface point.  Output [4 K][H][W] fp32, planar.
 // One thread per pixel: 5 depth loads (L1), 4 K coalesced plane stores = 16 K bytes per pixel written: HBM-bound.
-// IEEE operations in the oracle's order (plain intrinsics; sqrt and divisions are a handful per pixel).
+// IEEE operations in the oracle's order; the ~25 divisions and 2 + K square roots per pixel are what the kernel's time
+// goes to, so they run as the branch-free fast paths wherever their operands are mid-range (see div_ieee below).
 #include "ggt_internal.h"
+#include "ggt_packed.cuh"
 
 namespace {
 
@@ -21,13 +23,21 @@ __device__ __forceinline__ V3 rt_mul(const float* R, V3 q) {
             fmaf(R[8], q.z, fmaf(R[5], q.y, __fmul_rn(R[2], q.x)))};
 }
 
+// IEEE a / b and sqrt(x): the branch-free fast paths of ggt_packed.cuh (verified bit for bit by ggt_selftest_arith) where
+// every operand and result is a normal number far from the exponent limits, the compiler's intrinsics otherwise.
+__device__ __forceinline__ bool mid(float x) { return x >= 1e-30f && x <= 1e30f; }
+__device__ __forceinline__ float div_ieee(float a, float b, bool fast) { return fast ? div1_neg(-a, b) : __fdiv_rn(a, b); }
+// v / |v| given l = |v| and whether l is mid-range: |v_i| <= l, so each quotient is 0 or a normal number
+__device__ __forceinline__ V3 unit3(V3 v, float l, bool fast) { return {div_ieee(v.x, l, fast), div_ieee(v.y, l, fast), div_ieee(v.z, l, fast)}; }
+__device__ __forceinline__ float sqrt_ieee(float x, bool fast) { return fast ? sqrt1(x) : __fsqrt_rn(x); }
+
 __device__ __forceinline__ float depth_at(const GgtFeatureParams& p, int u, int v) {
     if (u < 0 || v < 0 || u >= p.W || v >= p.H) return 0.0f;
     return __ldg(p.depth + (size_t)v * p.W + u);
 }
 __device__ __forceinline__ V3 cam_point(const GgtFeatureParams& p, int u, int v, float d) {
     const float uc = __fadd_rn((float)u, 0.5f), vc = __fadd_rn((float)v, 0.5f);
-    return {__fmul_rn(d, __fdiv_rn(__fsub_rn(uc, p.cx), p.fx)), __fmul_rn(d, __fdiv_rn(__fsub_rn(vc, p.cy), p.fy)), d};
+    return {__fmul_rn(d, div_ieee(__fsub_rn(uc, p.cx), p.fx, p.fast_ok != 0)), __fmul_rn(d, div_ieee(__fsub_rn(vc, p.cy), p.fy, p.fast_ok != 0)), d};
 }
 // difference along one axis: central where both neighbours have depth, else one-sided, else undefined
 __device__ __forceinline__ bool diff_axis(const GgtFeatureParams& p, int u, int v, int du, int dv, V3 centre, V3& out) {
@@ -61,8 +71,8 @@ k_features(const __grid_constant__ GgtFeatureParams p) {
             const float l2 = dot3(c, c);
             ok = l2 > 0.0f;
             if (ok) {
-                const float l = __fsqrt_rn(l2);
-                const V3 nc = {__fdiv_rn(c.x, l), __fdiv_rn(c.y, l), __fdiv_rn(c.z, l)};
+                const bool f = mid(l2);
+                const V3 nc = unit3(c, sqrt_ieee(l2, f), f);
                 n = rt_mul(p.R, nc);
                 P = rt_mul(p.R, sub3(pc, V3{p.t[0], p.t[1], p.t[2]}));
             }
@@ -70,18 +80,22 @@ k_features(const __grid_constant__ GgtFeatureParams p) {
     }
     if (ok) {
         const V3 dt = sub3(P, V3{p.Ct[0], p.Ct[1], p.Ct[2]});
-        const float l = __fsqrt_rn(dot3(dt, dt));
+        const float l2 = dot3(dt, dt);
+        const bool f = mid(l2);
+        const float l = sqrt_ieee(l2, f);
         ok = l > 0.0f;
-        if (ok) rt = {__fdiv_rn(dt.x, l), __fdiv_rn(dt.y, l), __fdiv_rn(dt.z, l)};
+        if (ok) rt = unit3(dt, l, f);
     }
     const size_t plane = (size_t)p.W * p.H;
     for (int k = 0; k < p.n_views; ++k) {
         float f5 = 0.0f, f6 = 0.0f;
         if (ok) {
             const V3 dk = sub3(P, V3{p.v[k].C[0], p.v[k].C[1], p.v[k].C[2]});
-            const float l = __fsqrt_rn(dot3(dk, dk));
+            const float l2 = dot3(dk, dk);
+            const bool f = mid(l2);
+            const float l = sqrt_ieee(l2, f);
             if (l > 0.0f) {
-                const V3 rk = {__fdiv_rn(dk.x, l), __fdiv_rn(dk.y, l), __fdiv_rn(dk.z, l)};
+                const V3 rk = unit3(dk, l, f);
                 f5 = dot3(rk, n);                                              // item 5
                 f6 = dot3(rk, rt);                                             // item 6
             }

@@ -85,7 +85,8 @@ struct GgtFeatureView {
 };
 
 struct GgtFeatureParams {   // ggt_guidance_features (A.4 items 5-8)
-    int32_t W, H, n_views, pad_;
+    int32_t W, H, n_views;
+    int32_t fast_ok;       // fx, fy mid-range: the branch-free division is exact for (uc - cx) / fx
     float fx, fy, cx, cy;
     float R[9], t[3], Ct[3];
     const float* depth;

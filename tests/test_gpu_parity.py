@@ -55,6 +55,11 @@ def test_fast_reciprocal_and_division():
     b = torch.rand(1 << 24, generator=g, device="cuda") * 16 + 0.05
     a = (torch.rand(1 << 24, generator=g, device="cuda") * 2 - 1) * b * 0.25
     assert ctx.ggt_selftest_arith(a, b) == (0, 0, 0, 0)
+    # quotients up to magnitude 1 (unit vectors: |v_i| <= |v|), denominators over 12 decades
+    b = torch.exp(torch.rand(1 << 24, generator=g, device="cuda") * 28.0 - 14.0)
+    a = (torch.rand(1 << 24, generator=g, device="cuda") * 2 - 1) * b
+    a[::5] = b[::5]
+    assert ctx.ggt_selftest_arith(a, b) == (0, 0, 0, 0)
     # the ranges Eq. 11-12 sees: nu in [1e-16, 49 * clip^2], nu / 49, its square root
     b = torch.exp(torch.rand(1 << 24, generator=g, device="cuda") * 34.0 - 37.0)            # 1e-16 .. 0.05
     a = torch.full_like(b, 0.001)
