@@ -230,8 +230,10 @@ int ggt_volume_bind(ggt_ctx* ctx, const ggt_volume_desc* desc, void* dev_storage
     const int Dpad = v->n_groups * v->group;
     std::vector<float> tab(2 * (size_t)Dpad);
     for (int j = 0; j < Dpad; ++j) {
+        // bins >= D pad the last 128-bit group: z repeats the last plane, tau = -1e30 puts every sample of a padded
+        // bin behind the cut (s < -tau always), so the padding stays unobserved (T = 0, W = 0) whatever the geometry
         tab[j] = v->z[j < D ? j : D - 1];
-        tab[Dpad + j] = v->tau[j < D ? j : D - 1];
+        tab[Dpad + j] = j < D ? v->tau[j] : -1e30f;
     }
     cudaError_t e = cudaMemcpy(v->dev_tables, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { delete v; return cuda_fail(ctx, e, "upload of bin tables"); }
