@@ -216,3 +216,27 @@ def test_T14_misses():
     a = oracle.raymarch(tgt, views, const_maps(views, 2.0), NEAR, FAR, tau=TAU)[0]
     b = oracle.raymarch(tgt, views[::-1], const_maps(views, 2.0), NEAR, FAR, tau=TAU)[0]
     assert np.max(np.abs(a - b)) <= 1e-5
+
+
+def test_defaults_are_the_papers_constants():
+    """The defaults of the oracle's raymarch / temporal weight and of the binding are the constants the paper prints
+    (tests/golden/paper_constants.txt, each with its citation)."""
+    import inspect
+    import os
+    from paper_2505_18932_b200 import binding
+    gold = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_constants.txt")) as fh:
+        for line in fh:
+            line = line.split("#")[0].split()
+            if len(line) == 2:
+                gold[line[0]] = float(line[1])
+    o = inspect.signature(oracle.raymarch).parameters
+    b = inspect.signature(binding.Context.ggt_raymarch_depth).parameters
+    for sig in (o, b):
+        assert sig["tau"].default == gold["tau_metric"]
+        assert sig["step_scale"].default == gold["step_scale"]
+        assert sig["n_bisect"].default == gold["n_bisect"]
+    assert b["w_window"].default == gold["w_window"] and b["w_sigma0"].default == gold["w_sigma0"]
+    assert b["w_clip"].default == gold["tau_metric"]          # Eq. 12's clip is the paper's tau
+    assert inspect.signature(oracle.temporal_weight).parameters["eta"].default == gold["eta"]
+    assert inspect.signature(binding.Context.ggt_temporal_weight).parameters["eta"].default == gold["eta"]
