@@ -418,6 +418,23 @@ def main():
         e2e["pipelined"] = {"value": red_p["units"] / (red_p["ms"] / 1e3) / 1e9, "unit": UNIT, "ms_per_step": red_p["ms"] / e2e_steps,
                             "note": "same per-step copies, no host synchronise between steps (throughput of an online stream)"}
 
+    # ---- C5 only: the same frame with the zero-crossing search fused into the batch (no volume re-read) ---------
+    extra_multi = {}
+    if rank == 0 and inp.multi:
+        ids = inp.view_ids
+        d8 = [torch.empty_like(dev.depth) for _ in inp.targets]
+        c8 = [torch.empty_like(dev.conf) for _ in inp.targets]
+
+        def fused_frame():
+            dev.ctx.ggt_refine_depth_batch([dev.rgb_by[1][v] for v in ids], [dev.rgb_by[0][v] for v in ids],
+                                           [dev.depth_by[1][v] for v in ids], [dev.state_by[v] for v in ids], **REFINE)
+            dev.ctx.ggt_integrate_extract_batch(dev.vols, inp.targets, dev.rig_views, [dev.state_by[v] for v in ids],
+                                                dev.view_index, dev.flags, depth=d8, conf=c8)
+        kf = max(3, min(args.steps, 10))
+        ms_ff = timed(torch, None, fused_frame, kf, 2) / kf
+        extra_multi["fused_batch_frame"] = {"call": "ggt_refine_depth_batch + ggt_integrate_extract_batch (8 targets, no volume re-read)",
+                                            "ms_per_frame": ms_ff}
+
     # ---- extra legs (not the headline): fused integrate+extract, and the paper's own volume-free schedule ------
     extra = {}
     if rank == 0 and not inp.multi:
@@ -504,7 +521,7 @@ def main():
                 "integrate_gvoxel_view_per_s": inp.vv_per_step / len(inp.targets) / (integ_ms / 1e3) / 1e9 if integ_ms > 0 else None,
                 "ms_per_target": ms_per_step / len(inp.targets),
                 "paper_context": "PAPER.md Table 4: TSDF stage 6 ms/frame at 1352x1014, K=4, GPU not stated",
-                "extra": extra}
+                "extra": extra if not inp.multi else extra_multi}
         if not args.no_cpu_baseline and world == 1 and not inp.multi:
             line["cpu_baseline"] = cpu_baseline(inp)
         print(json.dumps(line))

@@ -172,6 +172,13 @@ int ggt_integrate_batch(ggt_ctx* ctx, int32_t n_targets, ggt_volume* const* vols
                         int32_t n_rig_views, const ggt_camera* rig_views, const float* const* dev_depths,
                         int32_t n_views, const int32_t* view_index, uint32_t flags, void* stream);
 
+/* The batch with the zero-crossing search fused in (ggt_integrate_extract per target): dev_depth / dev_conf / dev_bin
+ * are HOST arrays of n_targets DEVICE pointers (arrays or entries may be NULL). */
+int ggt_integrate_extract_batch(ggt_ctx* ctx, int32_t n_targets, ggt_volume* const* vols, const ggt_camera* targets,
+                                int32_t n_rig_views, const ggt_camera* rig_views, const float* const* dev_depths,
+                                int32_t n_views, const int32_t* view_index, uint32_t flags, float* const* dev_depth,
+                                float* const* dev_conf, int32_t* const* dev_bin, void* stream);
+
 /* ---- step a7: zero-crossing depth (reading P13) ------------------------------------- */
 /* Outputs are fp32 / int32 H_t x W_t; any may be NULL.  Miss: depth 0, conf 0, bin -1. */
 int ggt_extract_depth(ggt_ctx* ctx, const ggt_volume* vol, float* dev_depth, float* dev_conf,

@@ -24,7 +24,7 @@ GGT_PROFILE_STAGES = 5
 EXPORTS = [
     "ggt_create", "ggt_destroy", "ggt_last_error", "ggt_launch_count", "ggt_profile_enable", "ggt_profile_collect", "ggt_selftest_arith", "ggt_workspace_bytes", "ggt_set_workspace",
     "ggt_volume_bytes", "ggt_volume_bind", "ggt_volume_unbind", "ggt_volume_reset", "ggt_volume_export",
-    "ggt_volume_tables", "ggt_refine_depth", "ggt_refine_depth_batch", "ggt_integrate", "ggt_integrate_batch", "ggt_extract_depth", "ggt_integrate_extract",
+    "ggt_volume_tables", "ggt_refine_depth", "ggt_refine_depth_batch", "ggt_integrate", "ggt_integrate_batch", "ggt_integrate_extract_batch", "ggt_extract_depth", "ggt_integrate_extract",
     "ggt_raymarch_depth", "ggt_guidance_features", "ggt_temporal_weight", "ggt_integrate_weighted", "ggt_raymarch_depth_weighted",
     "ggt_frame_staging_bytes", "ggt_frame_host",
 ]
@@ -110,6 +110,9 @@ def load_library() -> ctypes.CDLL:
                                            ctypes.POINTER(ggt_refine_params), vp]
     lib.ggt_integrate_batch.argtypes = [vp, i32, ctypes.POINTER(vp), camp, i32, camp, ctypes.POINTER(vp), i32,
                                         ctypes.POINTER(i32), u32, vp]
+    lib.ggt_integrate_extract_batch.argtypes = [vp, i32, ctypes.POINTER(vp), camp, i32, camp, ctypes.POINTER(vp), i32,
+                                                ctypes.POINTER(i32), u32, ctypes.POINTER(vp), ctypes.POINTER(vp),
+                                                ctypes.POINTER(vp), vp]
     lib.ggt_frame_staging_bytes.argtypes = [descp, i32, i32, i32, i32]
     lib.ggt_frame_staging_bytes.restype = ctypes.c_size_t
     lib.ggt_frame_host.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), ctypes.POINTER(vp),
@@ -265,6 +268,23 @@ class Context:
         idx = (ctypes.c_int32 * (T * V))(*[int(i) for row in view_index for i in row])
         rc = self.lib.ggt_integrate_batch(self.h, T, varr, tarr, R, rarr, ptrs, V, idx, flags, _stream())
         self.check(rc, "ggt_integrate_batch")
+
+    def ggt_integrate_extract_batch(self, vols, targets, rig_views, depths, view_index, flags=GGT_OVERWRITE, depth=None,
+                                    conf=None, bins=None):
+        """ggt_integrate_batch with the zero-crossing search fused in; depth / conf / bins: lists of tensors (or None)."""
+        T, R = len(targets), len(rig_views)
+        V = len(view_index[0])
+        tarr = (ggt_camera * T)(*[to_camera(c) for c in targets])
+        rarr = (ggt_camera * R)(*[to_camera(c) for c in rig_views])
+        varr = (ctypes.c_void_p * T)(*[v.h for v in vols])
+        ptrs = (ctypes.c_void_p * R)(*[d.data_ptr() for d in depths])
+        idx = (ctypes.c_int32 * (T * V))(*[int(i) for row in view_index for i in row])
+
+        def arr(lst):
+            return None if lst is None else (ctypes.c_void_p * T)(*[None if t is None else t.data_ptr() for t in lst])
+        rc = self.lib.ggt_integrate_extract_batch(self.h, T, varr, tarr, R, rarr, ptrs, V, idx, flags, arr(depth), arr(conf),
+                                                  arr(bins), _stream())
+        self.check(rc, "ggt_integrate_extract_batch")
 
     def ggt_integrate_extract(self, vol: "Volume", target, views, depths, flags=GGT_OVERWRITE, depth=None,
                               conf=None, bins=None):

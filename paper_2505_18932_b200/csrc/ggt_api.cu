@@ -473,9 +473,11 @@ int ggt_integrate_extract(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
     return integrate_impl(ctx, vol, target, n_views, views, dev_depths, nullptr, flags, true, dev_depth, dev_conf, dev_bin, stream);
 }
 
-int ggt_integrate_batch(ggt_ctx* ctx, int32_t n_targets, ggt_volume* const* vols, const ggt_camera* targets,
-                        int32_t n_rig_views, const ggt_camera* rig_views, const float* const* dev_depths,
-                        int32_t n_views, const int32_t* view_index, uint32_t flags, void* stream) {
+static int integrate_batch_impl(ggt_ctx* ctx, int32_t n_targets, ggt_volume* const* vols, const ggt_camera* targets,
+                                int32_t n_rig_views, const ggt_camera* rig_views, const float* const* dev_depths,
+                                int32_t n_views, const int32_t* view_index, uint32_t flags, bool fused,
+                                float* const* dev_depth_out, float* const* dev_conf_out, int32_t* const* dev_bin_out,
+                                void* stream) {
     if (!ctx) return GGT_ERR_INVALID_ARG;
     if (!vols || !targets || !rig_views || !dev_depths || !view_index) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL argument to ggt_integrate_batch");
     if (n_targets < 1) return fail(ctx, GGT_ERR_SHAPE, "n_targets %d", n_targets);
@@ -510,17 +512,37 @@ int ggt_integrate_batch(ggt_ctx* ctx, int32_t n_targets, ggt_volume* const* vols
         p.accumulate = flags == GGT_ACCUMULATE ? 1 : 0;
         p.decay = vol->desc.decay; p.cap = vol->desc.weight_cap;
         p.tables = vol->dev_tables; p.voxels = vol->dev_voxels;
+        if (fused) {
+            p.depth = dev_depth_out ? dev_depth_out[t] : nullptr;
+            p.conf = dev_conf_out ? dev_conf_out[t] : nullptr;
+            p.bin = dev_bin_out ? dev_bin_out[t] : nullptr;
+        }
         for (int k = 0; k < n_views; ++k) {
             const int idx = view_index[t * n_views + k];
             fill_view_params(targets[t], rig_views[idx], maps[idx], p.v[k]);
         }
         detect_fast_paths(p, n_views);
         StageTimer tm(ctx, GGT_STAGE_INTEGRATE, st);
-        cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, false, st);
+        cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, fused, st);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "integrate launch");
         ctx->launches += 1;
     }
     return GGT_OK;
+}
+
+int ggt_integrate_batch(ggt_ctx* ctx, int32_t n_targets, ggt_volume* const* vols, const ggt_camera* targets,
+                        int32_t n_rig_views, const ggt_camera* rig_views, const float* const* dev_depths,
+                        int32_t n_views, const int32_t* view_index, uint32_t flags, void* stream) {
+    return integrate_batch_impl(ctx, n_targets, vols, targets, n_rig_views, rig_views, dev_depths, n_views, view_index, flags,
+                                false, nullptr, nullptr, nullptr, stream);
+}
+
+int ggt_integrate_extract_batch(ggt_ctx* ctx, int32_t n_targets, ggt_volume* const* vols, const ggt_camera* targets,
+                                int32_t n_rig_views, const ggt_camera* rig_views, const float* const* dev_depths,
+                                int32_t n_views, const int32_t* view_index, uint32_t flags, float* const* dev_depth,
+                                float* const* dev_conf, int32_t* const* dev_bin, void* stream) {
+    return integrate_batch_impl(ctx, n_targets, vols, targets, n_rig_views, rig_views, dev_depths, n_views, view_index, flags,
+                                true, dev_depth, dev_conf, dev_bin, stream);
 }
 
 int ggt_extract_depth(ggt_ctx* ctx, const ggt_volume* vol, float* dev_depth, float* dev_conf, int32_t* dev_bin,

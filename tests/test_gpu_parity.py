@@ -374,5 +374,25 @@ def test_integrate_batch_equals_per_target_calls():
         Tb, Wb = b.ggt_volume_export()
         assert torch.equal(Ta, Tb) and torch.equal(Wa, Wb)
     assert float((Wa > 0).float().mean()) > 0.1
+    # the fused batch gives the same volumes plus what ggt_extract_depth gives on each of them
+    ctx_c = binding.Context()
+    vc = mk(ctx_c)
+    for v in vc:
+        v.ggt_volume_reset()
+    n = targets[0].width * targets[0].height
+    outs = [[torch.empty(n, device="cuda") for _ in targets] for _ in range(2)]
+    bins = [torch.empty(n, dtype=torch.int32, device="cuda") for _ in targets]
+    for f in range(2):
+        dep = {v: torch.from_numpy(wl.view_inputs(f, v)[0]).cuda() for v in ids}
+        ctx_c.ggt_integrate_extract_batch(vc, targets, rig_views, [dep[v] for v in ids], [[pos[v] for v in vi] for vi in vis],
+                                          binding.GGT_ACCUMULATE, depth=outs[0], conf=outs[1], bins=bins)
+    torch.cuda.synchronize()
+    for t, (c, b) in enumerate(zip(vc, vb)):
+        Tc, Wc = c.ggt_volume_export()
+        Tb, Wb = b.ggt_volume_export()
+        assert torch.equal(Tc, Tb) and torch.equal(Wc, Wb)
+        d, cf, bn = torch.empty(n, device="cuda"), torch.empty(n, device="cuda"), torch.empty(n, dtype=torch.int32, device="cuda")
+        ctx_b.ggt_extract_depth(b, d, cf, bn)
+        assert torch.equal(d, outs[0][t]) and torch.equal(cf, outs[1][t]) and torch.equal(bn, bins[t])
     with pytest.raises(binding.GgtError):
         ctx_a.ggt_integrate_batch(va, targets, rig_views, [dep[v] for v in ids], [[99] * len(vis[0])] * len(targets))
