@@ -2,34 +2,43 @@
 // reading P13: first bin pair with T_j > 0 >= T_{j+1} and both weights > 0; linear interpolation in z;
 // confidence = interpolated weight), plus the canonical-layout export used by the tests.
 //
-// One thread per target ray.  The volume layout [group][v][u][G][{T,W}] makes every load a 128-bit word and
-// every warp request 512 contiguous bytes.  Loads are issued UNROLL groups ahead; after each batch a warp
-// vote (__all_sync) ends the march for the warp once all 32 rays have their crossing, so the kernel reads
-// the volume only up to the front-most surface instead of all of it.
+// One thread per target ray.  The volume is two planes per group, [group][v][u] x {G values of T} and the same for
+// W: the search reads the T plane only (64-bit words, 256 contiguous bytes per warp request), UNROLL groups ahead,
+// and fetches weights just for the candidates; after each batch a warp vote (__all_sync) ends the march for the warp
+// once all 32 rays have their crossing, so the kernel reads at most half of the volume, up to the front-most surface.
 #include "ggt_internal.h"
 
 namespace {
 
+// G values of one plane word (T or W) of a group
 template <bool HALF>
-__device__ __forceinline__ void unpack(const uint4& w, float* T, float* Wv) {
+__device__ __forceinline__ void unpack(const uint2& w, float* x) {
     if (HALF) {
-        const uint32_t a[4] = {w.x, w.y, w.z, w.w};
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&a[i]));
-            T[i] = f.x; Wv[i] = f.y;
-        }
+        const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&w.x));
+        const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&w.y));
+        x[0] = a.x; x[1] = a.y; x[2] = b.x; x[3] = b.y;
     } else {
-        T[0] = __uint_as_float(w.x); Wv[0] = __uint_as_float(w.y);
-        T[1] = __uint_as_float(w.z); Wv[1] = __uint_as_float(w.w);
+        x[0] = __uint_as_float(w.x); x[1] = __uint_as_float(w.y);
     }
+}
+
+// W of bin j of this ray (a rare, on-demand load from the W plane)
+template <bool HALF>
+__device__ __forceinline__ float weight_at(const uint2* wplane, size_t plane, int j) {
+    constexpr int G = HALF ? 4 : 2;
+    float x[G];
+    unpack<HALF>(__ldg(wplane + (size_t)(j / G) * plane), x);
+    float r = x[0];
+#pragma unroll
+    for (int i = 1; i < G; ++i) r = (j % G) == i ? x[i] : r;
+    return r;
 }
 
 template <bool HALF>
 __global__ void __launch_bounds__(256)
 k_extract(const __grid_constant__ GgtExtractParams p) {
     constexpr int G = HALF ? 4 : 2;
-    constexpr int UNROLL = 4;
+    constexpr int UNROLL = 8;                            // 64-bit loads in flight per thread
     extern __shared__ float s_z[];                       // z[Dpad]
     const int Dpad = p.n_groups * G;
     for (int i = threadIdx.y * 32 + threadIdx.x; i < Dpad; i += 256) s_z[i] = __ldg(p.tables + i);
@@ -39,35 +48,40 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
     if (v >= p.Ht) return;                               // whole warp leaves together (one row per warp)
     const bool live = u < p.Wt;
     const size_t plane = (size_t)p.Wt * p.Ht;
-    const uint4* vox = reinterpret_cast<const uint4*>(p.voxels) + ((size_t)v * p.Wt + (live ? u : 0));
+    const uint2* tpl = reinterpret_cast<const uint2*>(p.voxels) + ((size_t)v * p.Wt + (live ? u : 0));   // T plane
+    const uint2* wpl = tpl + (size_t)p.n_groups * plane;                                                  // W plane
 
+    // The search runs on the T plane alone (half of the volume's bytes): a candidate is T_{j-1} > 0 >= T_j; only then
+    // are the two weights fetched, and the candidate is a crossing if both bins were observed (reading P13).  An
+    // unobserved bin holds T = 0, so it ends a positive run as a candidate and is then rejected by its W = 0.
     bool found = !live;
-    float pT = 0.0f, pW = 0.0f, pz = 0.0f;
+    float pT = 0.0f, pz = 0.0f;
     float out_d = 0.0f, out_c = 0.0f;
     int out_b = -1;
     for (int g = 0; g < p.n_groups; g += UNROLL) {
-        uint4 w[UNROLL];
+        uint2 w[UNROLL];
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q)
-            w[q] = (g + q < p.n_groups && !found) ? __ldcs(vox + (size_t)(g + q) * plane) : make_uint4(0, 0, 0, 0);
+            w[q] = (g + q < p.n_groups && !found) ? __ldcs(tpl + (size_t)(g + q) * plane) : make_uint2(0, 0);
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q) {
-            float T[G], Wv[G];
-            unpack<HALF>(w[q], T, Wv);
+            float T[G];
+            unpack<HALF>(w[q], T);
 #pragma unroll
             for (int i = 0; i < G; ++i) {
                 const int j = (g + q) * G + i;
                 const float z = s_z[min(j, Dpad - 1)];
-                const bool hit = !found && (j > 0) && (j < p.D) && (pW > 0.0f) && (Wv[i] > 0.0f) && (pT > 0.0f) &&
-                                 !(T[i] > 0.0f);
-                if (hit) {
-                    const float f = __fdiv_rn(pT, __fsub_rn(pT, T[i]));
-                    out_d = fmaf(f, __fsub_rn(z, pz), pz);
-                    out_c = fmaf(f, __fsub_rn(Wv[i], pW), pW);
-                    out_b = j - 1;
-                    found = true;
+                if (!found && pT > 0.0f && !(T[i] > 0.0f) && j < p.D) {
+                    const float Wa = weight_at<HALF>(wpl, plane, j - 1), Wb = weight_at<HALF>(wpl, plane, j);
+                    if (Wa > 0.0f && Wb > 0.0f) {
+                        const float f = __fdiv_rn(pT, __fsub_rn(pT, T[i]));
+                        out_d = fmaf(f, __fsub_rn(z, pz), pz);
+                        out_c = fmaf(f, __fsub_rn(Wb, Wa), Wa);
+                        out_b = j - 1;
+                        found = true;
+                    }
                 }
-                pT = T[i]; pW = Wv[i]; pz = z;
+                pT = T[i]; pz = z;
             }
         }
         if (__all_sync(0xffffffffu, found)) break;
@@ -88,10 +102,12 @@ k_export(GgtExtractParams p, float* __restrict__ T_out, float* __restrict__ W_ou
     if (u >= p.Wt || v >= p.Ht) return;
     const size_t plane = (size_t)p.Wt * p.Ht;
     const size_t ray = (size_t)v * p.Wt + u;
-    const uint4* vox = reinterpret_cast<const uint4*>(p.voxels) + ray;
+    const uint2* tpl = reinterpret_cast<const uint2*>(p.voxels) + ray;
+    const uint2* wpl = tpl + (size_t)p.n_groups * plane;
     for (int g = 0; g < p.n_groups; ++g) {
         float T[G], Wv[G];
-        unpack<HALF>(vox[(size_t)g * plane], T, Wv);
+        unpack<HALF>(tpl[(size_t)g * plane], T);
+        unpack<HALF>(wpl[(size_t)g * plane], Wv);
         for (int i = 0; i < G; ++i) {
             const int j = g * G + i;
             if (j < p.D) {
