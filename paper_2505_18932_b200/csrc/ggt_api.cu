@@ -94,7 +94,7 @@ size_t header_bytes_of(const ggt_volume_desc* d) {
 size_t voxel_bytes_of(const ggt_volume_desc* d) {
     const int G = ggt_group_of(d->dtype);
     const int ng = (d->bins + G - 1) / G;
-    return (size_t)ng * d->width * d->height * 16;
+    return (size_t)ng * d->width * d->height * 32;     // one 128-bit word per group and pixel in each of the two planes
 }
 
 }  // namespace

@@ -3,7 +3,8 @@
 // confidence = interpolated weight), plus the canonical-layout export used by the tests.
 //
 // One thread per target ray.  The volume is two planes per group, [group][v][u] x {G values of T} and the same for
-// W: the search reads the T plane only (64-bit words, 256 contiguous bytes per warp request), UNROLL groups ahead,
+// W (G = 4 bins fp32, 8 bins fp16): the search reads the T plane only (128-bit words, 512 contiguous bytes per warp
+// request), UNROLL groups ahead,
 // and fetches weights just for the candidates; after each batch a warp vote (__all_sync) ends the march for the warp
 // once all 32 rays have their crossing, so the kernel reads at most half of the volume, up to the front-most surface.
 #include "ggt_internal.h"
@@ -12,20 +13,23 @@ namespace {
 
 // G values of one plane word (T or W) of a group
 template <bool HALF>
-__device__ __forceinline__ void unpack(const uint2& w, float* x) {
+__device__ __forceinline__ void unpack(const uint4& w, float* x) {
     if (HALF) {
-        const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&w.x));
-        const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&w.y));
-        x[0] = a.x; x[1] = a.y; x[2] = b.x; x[3] = b.y;
+        const uint32_t c[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&c[i]));
+            x[2 * i] = f.x; x[2 * i + 1] = f.y;
+        }
     } else {
-        x[0] = __uint_as_float(w.x); x[1] = __uint_as_float(w.y);
+        x[0] = __uint_as_float(w.x); x[1] = __uint_as_float(w.y); x[2] = __uint_as_float(w.z); x[3] = __uint_as_float(w.w);
     }
 }
 
 // W of bin j of this ray (a rare, on-demand load from the W plane)
 template <bool HALF>
-__device__ __forceinline__ float weight_at(const uint2* wplane, size_t plane, int j) {
-    constexpr int G = HALF ? 4 : 2;
+__device__ __forceinline__ float weight_at(const uint4* wplane, size_t plane, int j) {
+    constexpr int G = HALF ? 8 : 4;
     float x[G];
     unpack<HALF>(__ldg(wplane + (size_t)(j / G) * plane), x);
     float r = x[0];
@@ -37,8 +41,8 @@ __device__ __forceinline__ float weight_at(const uint2* wplane, size_t plane, in
 template <bool HALF>
 __global__ void __launch_bounds__(256)
 k_extract(const __grid_constant__ GgtExtractParams p) {
-    constexpr int G = HALF ? 4 : 2;
-    constexpr int UNROLL = 8;                            // 64-bit loads in flight per thread
+    constexpr int G = HALF ? 8 : 4;
+    constexpr int UNROLL = 4;                            // 128-bit loads in flight per thread
     extern __shared__ float s_z[];                       // z[Dpad]
     const int Dpad = p.n_groups * G;
     for (int i = threadIdx.y * 32 + threadIdx.x; i < Dpad; i += 256) s_z[i] = __ldg(p.tables + i);
@@ -48,8 +52,8 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
     if (v >= p.Ht) return;                               // whole warp leaves together (one row per warp)
     const bool live = u < p.Wt;
     const size_t plane = (size_t)p.Wt * p.Ht;
-    const uint2* tpl = reinterpret_cast<const uint2*>(p.voxels) + ((size_t)v * p.Wt + (live ? u : 0));   // T plane
-    const uint2* wpl = tpl + (size_t)p.n_groups * plane;                                                  // W plane
+    const uint4* tpl = reinterpret_cast<const uint4*>(p.voxels) + ((size_t)v * p.Wt + (live ? u : 0));   // T plane
+    const uint4* wpl = tpl + (size_t)p.n_groups * plane;                                                  // W plane
 
     // The search runs on the T plane alone (half of the volume's bytes): a candidate is T_{j-1} > 0 >= T_j; only then
     // are the two weights fetched, and the candidate is a crossing if both bins were observed (reading P13).  An
@@ -59,10 +63,10 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
     float out_d = 0.0f, out_c = 0.0f;
     int out_b = -1;
     for (int g = 0; g < p.n_groups; g += UNROLL) {
-        uint2 w[UNROLL];
+        uint4 w[UNROLL];
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q)
-            w[q] = (g + q < p.n_groups && !found) ? __ldcs(tpl + (size_t)(g + q) * plane) : make_uint2(0, 0);
+            w[q] = (g + q < p.n_groups && !found) ? __ldcs(tpl + (size_t)(g + q) * plane) : make_uint4(0, 0, 0, 0);
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q) {
             float T[G];
@@ -96,14 +100,14 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
 template <bool HALF>
 __global__ void __launch_bounds__(256)
 k_export(GgtExtractParams p, float* __restrict__ T_out, float* __restrict__ W_out) {
-    constexpr int G = HALF ? 4 : 2;
+    constexpr int G = HALF ? 8 : 4;
     const int u = blockIdx.x * 32 + threadIdx.x;
     const int v = blockIdx.y * 8 + threadIdx.y;
     if (u >= p.Wt || v >= p.Ht) return;
     const size_t plane = (size_t)p.Wt * p.Ht;
     const size_t ray = (size_t)v * p.Wt + u;
-    const uint2* tpl = reinterpret_cast<const uint2*>(p.voxels) + ray;
-    const uint2* wpl = tpl + (size_t)p.n_groups * plane;
+    const uint4* tpl = reinterpret_cast<const uint4*>(p.voxels) + ray;
+    const uint4* wpl = tpl + (size_t)p.n_groups * plane;
     for (int g = 0; g < p.n_groups; ++g) {
         float T[G], Wv[G];
         unpack<HALF>(tpl[(size_t)g * plane], T);
@@ -122,7 +126,7 @@ k_export(GgtExtractParams p, float* __restrict__ T_out, float* __restrict__ W_ou
 
 cudaError_t ggt_launch_extract(const GgtExtractParams& p, int dtype, cudaStream_t st) {
     const dim3 blk(32, 8), grd((p.Wt + 31) / 32, (p.Ht + 7) / 8);
-    const int G = dtype == GGT_F16 ? 4 : 2;
+    const int G = dtype == GGT_F16 ? 8 : 4;
     const size_t smem = (size_t)p.n_groups * G * sizeof(float);
     if (dtype == GGT_F16) k_extract<true><<<grd, blk, smem, st>>>(p);
     else k_extract<false><<<grd, blk, smem, st>>>(p);

@@ -156,7 +156,7 @@ struct ggt_volume {
     void* dev_voxels = nullptr;    // inside the caller's storage
 };
 
-static inline int ggt_group_of(int dtype) { return dtype == GGT_F16 ? 4 : 2; }
+static inline int ggt_group_of(int dtype) { return dtype == GGT_F16 ? 8 : 4; }
 
 // ---- kernel launchers (each returns cudaError_t of the launch) ----------------------------------------
 cudaError_t ggt_launch_refine(int W, int H, const GgtRefineViews& tab, int stride, float lambda_t, float beta, float theta,
