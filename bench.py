@@ -131,7 +131,7 @@ class Inputs:
                                wl.storage, "persistent" if wl.persistent else "overwrite", wl.colour),
                 "targets_per_step": len(self.targets), "views": self.V, "bins": int(wl.z_bins.size),
                 "parallelism": "independent target streams per GPU x%d (no data-path collective)" % world,
-                "l2": "per-step traffic (volume %.2f GB written + read) exceeds the 126 MB L2; no explicit flush"
+                "l2": "per-step traffic (volume %.2f GB written, its T plane read back) exceeds the 126 MB L2; no explicit flush"
                       % (t.width * t.height * wl.z_bins.size * (4 if wl.storage == "f16" else 8) / 1e9)}
 
 
@@ -376,7 +376,8 @@ def main():
     integ_bytes = vox_bytes * (2 if wl.persistent else 1) + map_bytes      # algorithmic: DESIGN.md "Roofline"
     integ_ms = prof["integrate"][0] / max(prof["integrate"][1], 1)
     achieved = integ_bytes / (integ_ms / 1e3) / 1e9 if integ_ms > 0 else 0.0
-    path_bytes = (integ_bytes + (0 if args.fused else vox_bytes) + 2 * t.width * t.height * 4) * len(inp.targets)
+    # extract searches the T plane only (half of the volume) and fetches W for the crossing candidates
+    path_bytes = (integ_bytes + (0 if args.fused else vox_bytes // 2) + 2 * t.width * t.height * 4) * len(inp.targets)
     path_ms = stage_ms["integrate"] + stage_ms["extract"]
     roofline = {"bound": "hbm", "kernel": "k_integrate (ggt_integrate main kernel)", "achieved": achieved, "peak": hbm_peak,
                 "unit": "GB/s", "frac": achieved / hbm_peak, "traffic": None, "peak_source": peak_src,

@@ -59,7 +59,7 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
     // are the two weights fetched, and the candidate is a crossing if both bins were observed (reading P13).  An
     // unobserved bin holds T = 0, so it ends a positive run as a candidate and is then rejected by its W = 0.
     bool found = !live;
-    float pT = 0.0f, pz = 0.0f;
+    float pT = 0.0f;
     float out_d = 0.0f, out_c = 0.0f;
     int out_b = -1;
     for (int g = 0; g < p.n_groups; g += UNROLL) {
@@ -74,10 +74,10 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
 #pragma unroll
             for (int i = 0; i < G; ++i) {
                 const int j = (g + q) * G + i;
-                const float z = s_z[min(j, Dpad - 1)];
                 if (!found && pT > 0.0f && !(T[i] > 0.0f) && j < p.D) {
                     const float Wa = weight_at<HALF>(wpl, plane, j - 1), Wb = weight_at<HALF>(wpl, plane, j);
                     if (Wa > 0.0f && Wb > 0.0f) {
+                        const float pz = s_z[j - 1], z = s_z[j];
                         const float f = __fdiv_rn(pT, __fsub_rn(pT, T[i]));
                         out_d = fmaf(f, __fsub_rn(z, pz), pz);
                         out_c = fmaf(f, __fsub_rn(Wb, Wa), Wa);
@@ -85,7 +85,7 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
                         found = true;
                     }
                 }
-                pT = T[i]; pz = z;
+                pT = T[i];
             }
         }
         if (__all_sync(0xffffffffu, found)) break;
