@@ -42,7 +42,7 @@ template <bool HALF>
 __global__ void __launch_bounds__(256)
 k_extract(const __grid_constant__ GgtExtractParams p) {
     constexpr int G = HALF ? 8 : 4;
-    constexpr int UNROLL = 4;                            // 128-bit loads in flight per thread
+    constexpr int UNROLL = HALF ? 4 : 8;                 // 128-bit loads in flight per thread (measured: fp32 0.194 vs 0.206 ms at 8 vs 4; fp16 0.47 vs 0.36)
     extern __shared__ float s_z[];                       // z[Dpad]
     const int Dpad = p.n_groups * G;
     for (int i = threadIdx.y * 32 + threadIdx.x; i < Dpad; i += 256) s_z[i] = __ldg(p.tables + i);
