@@ -72,7 +72,7 @@ k_block_diff(int W, int H, int Wq, int Hq, const __grid_constant__ GgtRefineView
 
 __global__ void __launch_bounds__(256)
 k_mask_blend(int W, int H, int Wq, int Hq, const __grid_constant__ GgtRefineViews tab, float lambda_t, float beta,
-             float theta) {
+             float theta, int vec_ok) {
     const uint16_t* __restrict__ cq = tab.v[blockIdx.z].cq;
     const float* __restrict__ depth_cur = tab.v[blockIdx.z].depth_cur;
     float* __restrict__ depth_state = tab.v[blockIdx.z].depth_state;
@@ -129,7 +129,7 @@ k_mask_blend(int W, int H, int Wq, int Hq, const __grid_constant__ GgtRefineView
     const int yq1 = yq0 + 1 < Hq ? yq0 + 1 : Hq - 1;
     const int ly0 = yq0 - (y0q - 1), ly1 = yq1 - (y0q - 1);
     const size_t base = (size_t)y * W + xb;
-    const bool vec = (xb + 3 < W) && ((W & 3) == 0);
+    const bool vec = vec_ok && (xb + 3 < W);         // vec_ok: W % 4 == 0 and every depth / mask pointer 16-B aligned
     float dc[4], dp[4], out[4], mk[4];
     if (vec) {
         const float4 c4 = __ldg(reinterpret_cast<const float4*>(depth_cur + base));
@@ -203,7 +203,13 @@ cudaError_t ggt_launch_refine(int W, int H, const GgtRefineViews& tab, int strid
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     const dim3 grd2((W + TILE_W - 1) / TILE_W, (H + TILE_H - 1) / TILE_H, tab.n);
-    k_mask_blend<<<grd2, 256, 0, st>>>(W, H, Wq, Hq, tab, lambda_t, beta, theta);
+    // 128-bit accesses only when every row start is 16-B aligned: W % 4 == 0 and 16-B aligned caller pointers (a tensor
+    // view at a 4-byte offset is legal input and takes the scalar path)
+    uintptr_t bits = 0;
+    for (int k = 0; k < tab.n; ++k)
+        bits |= (uintptr_t)tab.v[k].depth_cur | (uintptr_t)tab.v[k].depth_state | (uintptr_t)tab.v[k].mask_out;
+    const int vec_ok = ((W & 3) == 0 && (bits & 15) == 0) ? 1 : 0;
+    k_mask_blend<<<grd2, 256, 0, st>>>(W, H, Wq, Hq, tab, lambda_t, beta, theta, vec_ok);
     *n_launches = 2;
     return cudaGetLastError();
 }

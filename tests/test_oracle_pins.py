@@ -379,6 +379,28 @@ def test_relative_transform_against_direct_projection():
         assert np.allclose(ref, got, rtol=2e-6, atol=2e-4)
 
 
+def test_tau_table_on_non_uniform_bins_hand_computed():
+    """orc_tau_table on bins that are NOT uniform (reading P3): tau_j = trunc_bins x the local
+    spacing (z[j+1] - z[j-1]) / 2, one-sided at the two ends.  Expected values are worked out by hand from the table
+    below (dyadic numbers, so every step is exact): a wrong central difference (e.g. z[j+1] - z[j], or a missing / 2),
+    a two-sided formula at the ends, or trunc_bins applied twice all fail."""
+    z = np.array([0.5, 0.625, 1.0, 1.125, 2.0, 4.0], np.float32)
+    #   spacings           one-sided 0.125 | (1.0-0.5)/2 | (1.125-0.625)/2 | (2-1)/2 | (4-1.125)/2 | one-sided 2.0
+    local = np.array([0.125, 0.25, 0.25, 0.5, 1.4375, 2.0], np.float32)
+    assert np.array_equal(oracle.tau_table(z, 2.0), 2.0 * local)
+    assert np.array_equal(oracle.tau_table(z, 1.5), np.array([0.1875, 0.375, 0.375, 0.75, 2.15625, 3.0], np.float32))
+    # trunc_metric > 0 overrides the spacing rule everywhere (PAPER.md:341, tau = 0.02 m)
+    assert np.array_equal(oracle.tau_table(z, 2.0, 0.02), np.full(6, np.float32(0.02)))
+    # inverse-depth bins of C2-C5: 1/z uniform, so z[j+1] - z[j-1] = 2 d z[j+1] z[j-1] with d the inverse-depth step;
+    # tau_j / (z[j+1] z[j-1]) must therefore be the constant 2 d in the interior (a one-sided difference z[j+1] - z[j]
+    # would give d z[j+1] z[j] instead: off by the ratio z[j] / z[j-1], up to 7 % here)
+    zi = synth.bins_inverse(0.5, 5.0, 64).astype(np.float64)
+    tau = oracle.tau_table(zi.astype(np.float32), 2.0).astype(np.float64)
+    d = (1.0 / 0.5 - 1.0 / 5.0) / 63
+    assert np.allclose(tau[1:-1] / (zi[2:] * zi[:-2]), 2.0 * d, rtol=2e-6)
+    assert np.isclose(tau[0], 2.0 * d * zi[0] * zi[1], rtol=2e-6) and np.isclose(tau[-1], 2.0 * d * zi[-1] * zi[-2], rtol=2e-6)
+
+
 # ------------------------------------------------------------------------------------------------
 # T8: behind-surface cut and clamp
 # ------------------------------------------------------------------------------------------------
