@@ -16,16 +16,17 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "ggt_oracle.cpp")
+_SRCS = [_SRC, os.path.join(_HERE, "ggt_oracle_splat.cpp")]
 _LIB = os.path.join(_HERE, "libggt_oracle.so")
 _lib = None
 
 
 def build(force: bool = False) -> str:
     """Compile the oracle (g++ -O2, contraction off, no fast-math)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(f) for f in _SRCS):
         tmp = _LIB + ".tmp%d" % os.getpid()
         subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
-                               "-o", tmp, _SRC])
+                               "-o", tmp] + _SRCS)
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -52,6 +53,8 @@ def _load():
         _lib = ctypes.CDLL(_LIB)
         _lib.orc_round_f16.restype = ctypes.c_float
         _lib.orc_round_f16.argtypes = [ctypes.c_float]
+        _lib.orc_exp_le0.restype = ctypes.c_float
+        _lib.orc_exp_le0.argtypes = [ctypes.c_float]
     return _lib
 
 
@@ -239,4 +242,61 @@ def features(target, depth, views: Sequence) -> np.ndarray:
     rc = lib.orc_features(ctypes.byref(t), _p(d, ctypes.c_float), ctypes.c_int32(V), cams, _p(out, ctypes.c_float))
     if rc != 0:
         raise ValueError("orc_features rc=%d" % rc)
+    return out
+
+
+# ---- f-3: forward warping with pixel-sized 3D Gaussians (ggt_oracle_splat.cpp) ---------------------------------------
+def exp_le0(q: float) -> float:
+    """The fp32 exponential both implementations use for alpha (reading S8), q <= 0."""
+    return float(_load().orc_exp_le0(ctypes.c_float(q)))
+
+
+def splat_project(target, view, u, v, D, sigma_px=0.5, dilation=0.3, z_cull=0.2):
+    """One Gaussian: (mu_x, mu_y, z, conic a, b, c, radius) or None if it is culled (readings S1-S3, S7)."""
+    lib = _load()
+    out = np.zeros(7, dtype=np.float32)
+    t, vw = _cam(target), _cam(view)
+    ok = lib.orc_splat_project(ctypes.byref(t), ctypes.byref(vw), ctypes.c_int32(int(u)), ctypes.c_int32(int(v)),
+                               ctypes.c_float(D), ctypes.c_float(sigma_px), ctypes.c_float(dilation),
+                               ctypes.c_float(z_cull), _p(out, ctypes.c_float))
+    return out if ok else None
+
+
+def splat_forward(target, view, depth, rgb=None, mask=None, sigma_px=0.5, dilation=0.3, z_cull=0.2):
+    """O-S. Returns dict(rgb (3,Ht,Wt) or None, alpha, depth, mask or None, count) of one view splatted into `target`."""
+    lib = _load()
+    H, W = int(view.height), int(view.width)
+    Ht, Wt = int(target.height), int(target.width)
+    depth = np.ascontiguousarray(depth, dtype=np.float32).reshape(H, W)
+    stride = 3
+    if rgb is not None:
+        rgb = np.ascontiguousarray(rgb, dtype=np.uint8)
+        stride = rgb.shape[2]
+    if mask is not None:
+        mask = np.ascontiguousarray(mask, dtype=np.float32).reshape(H, W)
+    o_rgb = np.empty((3, Ht, Wt), dtype=np.float32) if rgb is not None else None
+    o_alpha = np.empty((Ht, Wt), dtype=np.float32)
+    o_depth = np.empty((Ht, Wt), dtype=np.float32)
+    o_mask = np.empty((Ht, Wt), dtype=np.float32) if mask is not None else None
+    o_count = np.empty((Ht, Wt), dtype=np.int32)
+    t, vw = _cam(target), _cam(view)
+    rc = lib.orc_splat_forward(ctypes.byref(t), ctypes.byref(vw), _p(depth, ctypes.c_float), _p(rgb, ctypes.c_uint8),
+                               ctypes.c_int32(stride), _p(mask, ctypes.c_float), ctypes.c_float(sigma_px),
+                               ctypes.c_float(dilation), ctypes.c_float(z_cull), _p(o_rgb, ctypes.c_float),
+                               _p(o_alpha, ctypes.c_float), _p(o_depth, ctypes.c_float), _p(o_mask, ctypes.c_float),
+                               _p(o_count, ctypes.c_int32))
+    if rc != 0:
+        raise ValueError("orc_splat_forward rc=%d" % rc)
+    return dict(rgb=o_rgb, alpha=o_alpha, depth=o_depth, mask=o_mask, count=o_count)
+
+
+def temporal_weight_mask(prev_depth, prev_conf, novel_mask, beta=1.0, eta=15.0):
+    """Eq. 13 with a given novel-view mask M^t (the paper's splat-and-max), per pixel of D^{t-1}."""
+    lib = _load()
+    d = np.ascontiguousarray(prev_depth, dtype=np.float32)
+    c = np.ascontiguousarray(prev_conf, dtype=np.float32).reshape(d.shape)
+    m = np.ascontiguousarray(novel_mask, dtype=np.float32).reshape(d.shape)
+    out = np.empty_like(d)
+    lib.orc_temporal_weight_mask(ctypes.c_int64(d.size), _p(d, ctypes.c_float), _p(c, ctypes.c_float), _p(m, ctypes.c_float),
+                                 ctypes.c_float(beta), ctypes.c_float(eta), _p(out, ctypes.c_float))
     return out
