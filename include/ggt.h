@@ -256,6 +256,57 @@ int ggt_raymarch_depth_weighted(ggt_ctx* ctx, const ggt_camera* target, int32_t 
                                 const ggt_raymarch_params* params, float* dev_depth, float* dev_conf,
                                 int32_t* dev_steps, void* stream);
 
+/* ---- forward warping with pixel-sized 3D Gaussians -------------------------------------- */
+/* PAPER.md:63-65 (section 3.1): "for each pixel of an input I_k, we use the depth map D_k and pose to determine the 3D
+ * position of an isotropic, fully-opaque Gaussian.  The RGB color of each Gaussian is set to the underlying pixel value,
+ * and its scale is computed such that its projection in the source image I_k covers a single pixel.  This step produces
+ * a set of forward-rendered images along with accumulated opacity of the Gaussians, and depths in the novel view";
+ * PAPER.md:362-368 (A.3): the parameters are computed analytically; rendered with the 3D Gaussian
+ * splatting rasteriser the paper cites.  Readings S1-S8: 3D standard deviation sigma_px * D / fx of the
+ * source camera; EWA projection into the target (2D covariance sigma^2 J J^T + dilation I); alpha = min(0.99, exp(-1/2
+ * d^T Sigma'^-1 d)), a Gaussian contributes to a pixel iff alpha >= 1/255; per target pixel the contributors are
+ * composited front to back in ascending target depth (ties: ascending source pixel index) until the transmittance
+ * would fall below 1e-4; Gaussians with depth <= 0 or target depth < z_cull are dropped.  Paper / rasteriser values:
+ * sigma_px 0.5, dilation 0.3, z_cull 0.2.
+ *   target, view     HOST cameras (view = the input view whose pixels are splatted; sizes <= 32767)
+ *   dev_depth        DEVICE fp32 height x width z-depth of the view (<= 0 invalid), e.g. ggt_refine_depth's state
+ *   dev_rgb          DEVICE uint8 height x width x rgb_pixel_stride (3 or 4), may be NULL
+ *   dev_mask         DEVICE fp32 height x width (Eq. 1's M_k: ggt_refine_depth's dev_mask_out), may be NULL
+ *   dev_out_rgb      DEVICE fp32 [3][H_t][W_t], colour in source units (0..255), premultiplied by opacity, no background
+ *   dev_out_alpha    DEVICE fp32 H_t x W_t accumulated opacity 1 - T
+ *   dev_out_depth    DEVICE fp32 H_t x W_t opacity-normalised depth (0 where nothing landed)
+ *   dev_out_mask     DEVICE fp32 H_t x W_t the mask splatted like a colour channel
+ *   dev_out_count    DEVICE int32 H_t x W_t number of Gaussians with alpha >= 1/255 at the pixel (diagnostic)
+ * Every output may be NULL.  One call = one view (the paper renders the K views separately).
+ * Scratch is owned by the context and grows between calls (cudaMalloc, synchronising once per growth): 32 B per source
+ * pixel, 8 B per target pixel and 8 B per list entry; the list capacity is ggt_splat_reserve's, by default 40 entries per
+ * source pixel (a dense single surface needs about 20).  If a call needs more entries than the capacity, its outputs
+ * are zero and ggt_splat_status reports it: reserve what it asks for and call again.  Domain: views of comparable
+ * resolution (the sum of the Gaussians' footprints, in target pixels, must stay below 2^32).
+ * Errors: GGT_ERR_INVALID_ARG (NULL cameras / depth, parameter ranges), GGT_ERR_SHAPE (sizes), GGT_ERR_CUDA. */
+typedef struct ggt_splat_params {
+    float sigma_px;                /* > 0 */
+    float dilation;                /* >= 0 */
+    float z_cull;                  /* > 0 */
+    int32_t reserved;              /* 0 */
+} ggt_splat_params;
+int ggt_splat_forward(ggt_ctx* ctx, const ggt_camera* target, const ggt_camera* view, const float* dev_depth,
+                      const uint8_t* dev_rgb, int32_t rgb_pixel_stride, const float* dev_mask,
+                      const ggt_splat_params* params, float* dev_out_rgb, float* dev_out_alpha, float* dev_out_depth,
+                      float* dev_out_mask, int32_t* dev_out_count, void* stream);
+/* List capacity of later ggt_splat_forward calls, in entries (0 = the default rule). */
+int ggt_splat_reserve(ggt_ctx* ctx, int64_t entries);
+/* Synchronises `stream`; host_entries_last = list entries the last call produced, host_entries_needed = the largest
+ * number of entries any call since the last status query needed but did not have (0 = no call overflowed). */
+int ggt_splat_status(ggt_ctx* ctx, int64_t* host_entries_last, int64_t* host_entries_needed, void* stream);
+/* Eq. 13 with the paper's own novel-view mask: M^t = the channel-wise maximum of the n_masks
+ * splatted masks (ggt_splat_forward's dev_out_mask of each input view, rendered into the camera of D^{t-1});
+ * dev_weight_out = min(beta * omega_acc * max(1 - M^t, 0), eta) per pixel, 0 where depth or omega_acc is <= 0.
+ *   dev_masks   HOST array of n_masks (1..GGT_MAX_VIEWS) DEVICE pointers, each fp32 n_pixels */
+int ggt_temporal_weight_mask(ggt_ctx* ctx, int64_t n_pixels, const float* dev_prev_depth, const float* dev_prev_conf,
+                             int32_t n_masks, const float* const* dev_masks, float beta, float eta,
+                             float* dev_weight_out, void* stream);
+
 /* ---- network-input geometry features of the guidance depth --------------------- */
 /* PAPER.md:374-388 (A.4, items 5-8 of the blending network's input): per input view k and target pixel,
  *   (5) the dot product between the input-view ray direction and the normal of the TSDF depth D^t,

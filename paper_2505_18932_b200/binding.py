@@ -27,6 +27,7 @@ EXPORTS = [
     "ggt_volume_tables", "ggt_refine_depth", "ggt_refine_depth_batch", "ggt_integrate", "ggt_integrate_batch", "ggt_integrate_extract_batch", "ggt_extract_depth", "ggt_integrate_extract",
     "ggt_raymarch_depth", "ggt_guidance_features", "ggt_temporal_weight", "ggt_integrate_weighted", "ggt_raymarch_depth_weighted",
     "ggt_frame_staging_bytes", "ggt_frame_host",
+    "ggt_splat_forward", "ggt_splat_reserve", "ggt_splat_status", "ggt_temporal_weight_mask",
 ]
 
 
@@ -50,6 +51,11 @@ class ggt_raymarch_params(ctypes.Structure):
                 ("step_scale", ctypes.c_float), ("min_step", ctypes.c_float), ("max_evals", ctypes.c_int32),
                 ("n_bisect", ctypes.c_int32), ("w_sigma0", ctypes.c_float), ("w_clip", ctypes.c_float),
                 ("w_window", ctypes.c_int32)]
+
+
+class ggt_splat_params(ctypes.Structure):
+    _fields_ = [("sigma_px", ctypes.c_float), ("dilation", ctypes.c_float), ("z_cull", ctypes.c_float),
+                ("reserved", ctypes.c_int32)]
 
 
 class ggt_volume_desc(ctypes.Structure):
@@ -113,6 +119,11 @@ def load_library() -> ctypes.CDLL:
     lib.ggt_integrate_extract_batch.argtypes = [vp, i32, ctypes.POINTER(vp), camp, i32, camp, ctypes.POINTER(vp), i32,
                                                 ctypes.POINTER(i32), u32, ctypes.POINTER(vp), ctypes.POINTER(vp),
                                                 ctypes.POINTER(vp), vp]
+    lib.ggt_splat_forward.argtypes = [vp, camp, camp, vp, vp, i32, vp, ctypes.POINTER(ggt_splat_params), vp, vp, vp, vp, vp, vp]
+    lib.ggt_splat_reserve.argtypes = [vp, ctypes.c_int64]
+    lib.ggt_splat_status.argtypes = [vp, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64), vp]
+    lib.ggt_temporal_weight_mask.argtypes = [vp, ctypes.c_int64, vp, vp, i32, ctypes.POINTER(vp), ctypes.c_float, ctypes.c_float,
+                                             vp, vp]
     lib.ggt_frame_staging_bytes.argtypes = [descp, i32, i32, i32, i32]
     lib.ggt_frame_staging_bytes.restype = ctypes.c_size_t
     lib.ggt_frame_host.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), ctypes.POINTER(vp),
@@ -345,6 +356,33 @@ class Context:
         rc = self.lib.ggt_raymarch_depth_weighted(self.h, ctypes.byref(t), V, arr, ptrs, self._weight_ptrs(weights, V),
                                                   ctypes.byref(prm), _ptr(depth), _ptr(conf), _ptr(steps), _stream())
         self.check(rc, "ggt_raymarch_depth_weighted")
+
+    # ---- f-3: forward warping with pixel-sized 3D Gaussians --------------------------------------------
+    def ggt_splat_forward(self, target, view, depth, rgb=None, mask=None, out_rgb=None, out_alpha=None, out_depth=None,
+                          out_mask=None, out_count=None, sigma_px=0.5, dilation=0.3, z_cull=0.2):
+        t, arr = self._cams(target, [view])
+        stride = 3 if rgb is None else int(rgb.shape[2])
+        prm = ggt_splat_params(sigma_px, dilation, z_cull, 0)
+        rc = self.lib.ggt_splat_forward(self.h, ctypes.byref(t), arr, depth.data_ptr(), _ptr(rgb), stride, _ptr(mask),
+                                        ctypes.byref(prm), _ptr(out_rgb), _ptr(out_alpha), _ptr(out_depth), _ptr(out_mask),
+                                        _ptr(out_count), _stream())
+        self.check(rc, "ggt_splat_forward")
+
+    def ggt_splat_reserve(self, entries: int):
+        self.check(self.lib.ggt_splat_reserve(self.h, int(entries)), "ggt_splat_reserve")
+
+    def ggt_splat_status(self):
+        """(entries of the last call, entries needed by an overflowed call or 0); synchronises the current stream."""
+        last, need = ctypes.c_int64(), ctypes.c_int64()
+        self.check(self.lib.ggt_splat_status(self.h, ctypes.byref(last), ctypes.byref(need), _stream()), "ggt_splat_status")
+        return int(last.value), int(need.value)
+
+    def ggt_temporal_weight_mask(self, prev_depth, prev_conf, masks, weight_out, beta=1.0, eta=15.0):
+        K = len(masks)
+        ptrs = (ctypes.c_void_p * K)(*[m.data_ptr() for m in masks])
+        rc = self.lib.ggt_temporal_weight_mask(self.h, prev_depth.numel(), prev_depth.data_ptr(), prev_conf.data_ptr(), K, ptrs,
+                                               beta, eta, weight_out.data_ptr(), _stream())
+        self.check(rc, "ggt_temporal_weight_mask")
 
     # ---- f-4: network-input geometry features of the guidance depth ---------------------------------
     def ggt_guidance_features(self, target, depth, views, features):

@@ -19,7 +19,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libggt.so")
 # (source, extra defines)
 UNITS = [("ggt_api.cu", []), ("ggt_refine.cu", []), ("ggt_weight.cu", []), ("ggt_extract.cu", []),
-         ("ggt_raymarch.cu", []), ("ggt_temporal.cu", []), ("ggt_features.cu", [])] + \
+         ("ggt_raymarch.cu", []), ("ggt_temporal.cu", []), ("ggt_features.cu", []), ("ggt_splat.cu", [])] + \
         [("ggt_integrate.cu", ["-DGGT_INTEGRATE_VARIANT=%d" % v]) for v in range(4)]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--fmad=false", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math"]

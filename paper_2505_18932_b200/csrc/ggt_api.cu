@@ -130,6 +130,8 @@ int ggt_destroy(ggt_ctx* ctx) {
     ggt_ctx* c = ctx;
     if (c->ws_owned && c->ws) cudaFree(c->ws);
     if (c->cq) cudaFree(c->cq);
+    if (c->splat_ws) cudaFree(c->splat_ws);
+    if (c->splat_flags) cudaFree(c->splat_flags);
     for (auto& r : c->prof_pool) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     if (c->ev_inputs_free) cudaEventDestroy(c->ev_inputs_free);
     if (c->ev_h2d_done) cudaEventDestroy(c->ev_h2d_done);
@@ -625,6 +627,108 @@ int ggt_temporal_weight(ggt_ctx* ctx, const ggt_camera* prev_target, const float
     }
     cudaError_t e = ggt_launch_temporal_weight(p, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "temporal-weight launch");
+    ctx->launches += 1;
+    return GGT_OK;
+}
+
+// ---- f-3: forward warping with pixel-sized Gaussians ---------------------------------------------------------------
+int ggt_splat_reserve(ggt_ctx* ctx, int64_t entries) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    if (entries < 0 || entries > 0xfffffff0ll) return fail(ctx, GGT_ERR_INVALID_ARG, "entries %lld not in [0, 2^32)", (long long)entries);
+    ctx->splat_entries = (size_t)entries;
+    return GGT_OK;
+}
+
+int ggt_splat_status(ggt_ctx* ctx, int64_t* host_entries_last, int64_t* host_entries_needed, void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    uint32_t f[2] = {0, 0};
+    if (ctx->splat_flags) {
+        cudaStream_t st = (cudaStream_t)stream;
+        cudaError_t e = cudaMemcpyAsync(f, ctx->splat_flags, sizeof f, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemsetAsync(ctx->splat_flags + 1, 0, sizeof(uint32_t), st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "ggt_splat_status");
+    }
+    if (host_entries_last) *host_entries_last = f[0];
+    if (host_entries_needed) *host_entries_needed = f[1];
+    return GGT_OK;
+}
+
+int ggt_splat_forward(ggt_ctx* ctx, const ggt_camera* target, const ggt_camera* view, const float* dev_depth,
+                      const uint8_t* dev_rgb, int32_t rgb_pixel_stride, const float* dev_mask,
+                      const ggt_splat_params* params, float* dev_out_rgb, float* dev_out_alpha, float* dev_out_depth,
+                      float* dev_out_mask, int32_t* dev_out_count, void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    if (!target || !view || !dev_depth || !params) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL camera / depth / params pointer");
+    if (target->width <= 0 || target->height <= 0 || target->width > 32767 || target->height > 32767 || view->width <= 0 ||
+        view->height <= 0 || view->width > 32767 || view->height > 32767)
+        return fail(ctx, GGT_ERR_SHAPE, "view %dx%d / target %dx%d", view->width, view->height, target->width, target->height);
+    if (!(target->fx > 0.0f) || !(target->fy > 0.0f) || !(view->fx > 0.0f) || !(view->fy > 0.0f))
+        return fail(ctx, GGT_ERR_INVALID_ARG, "focal length");
+    if (dev_rgb && rgb_pixel_stride != 3 && rgb_pixel_stride != 4) return fail(ctx, GGT_ERR_INVALID_ARG, "rgb_pixel_stride %d (3 or 4)", rgb_pixel_stride);
+    if (!(params->sigma_px > 0.0f) || !(params->dilation >= 0.0f) || !(params->z_cull > 0.0f))
+        return fail(ctx, GGT_ERR_INVALID_ARG, "sigma_px / z_cull must be > 0, dilation >= 0");
+    const size_t N = (size_t)view->width * view->height, Nt = (size_t)target->width * target->height;
+    size_t cap = ctx->splat_entries ? ctx->splat_entries : 40 * N;
+    if (cap > 0xfffffff0ull) cap = 0xfffffff0ull;
+    const size_t n_blocks = (Nt + 2047) / 2048;
+    const size_t o_gauss = 0, o_counts = align_up(o_gauss + N * 32, 256), o_pos = align_up(o_counts + Nt * 4, 256),
+                 o_sums = align_up(o_pos + Nt * 4, 256), o_entries = align_up(o_sums + n_blocks * 4, 256),
+                 need = o_entries + cap * 8;
+    if (ctx->splat_ws_bytes < need) {            // grows between calls only (synchronises: cudaFree)
+        if (ctx->splat_ws) cudaFree(ctx->splat_ws);
+        ctx->splat_ws = nullptr; ctx->splat_ws_bytes = 0;
+        cudaError_t e = cudaMalloc(&ctx->splat_ws, need);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "splat scratch allocation");
+        ctx->splat_ws_bytes = need;
+    }
+    if (!ctx->splat_flags) {
+        cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&ctx->splat_flags), 2 * sizeof(uint32_t));
+        if (e == cudaSuccess) e = cudaMemset(ctx->splat_flags, 0, 2 * sizeof(uint32_t));
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "splat flags allocation");
+    }
+    GgtSplatParams p;
+    memset(&p, 0, sizeof p);
+    p.W = view->width; p.H = view->height; p.Wt = target->width; p.Ht = target->height;
+    p.rgb_stride = rgb_pixel_stride; p.capacity = (uint32_t)cap;
+    relative_transform(*view, *target, p.h, p.e);       // roles exchanged: from the view's pixel / depth into the target
+    p.fx_t = target->fx; p.fy_t = target->fy; p.cx_t = target->cx; p.cy_t = target->cy; p.fx_s = view->fx;
+    p.sigma_px = params->sigma_px; p.dilation = params->dilation; p.z_cull = params->z_cull;
+    p.depth = dev_depth; p.rgb = dev_rgb; p.mask = dev_mask;
+    char* w = static_cast<char*>(ctx->splat_ws);
+    p.gauss = reinterpret_cast<float*>(w + o_gauss);
+    p.counts = reinterpret_cast<uint32_t*>(w + o_counts);
+    p.pos = reinterpret_cast<uint32_t*>(w + o_pos);
+    p.block_sums = reinterpret_cast<uint32_t*>(w + o_sums);
+    p.entries = reinterpret_cast<uint2*>(w + o_entries);
+    p.total = ctx->splat_flags; p.overflow = ctx->splat_flags + 1;
+    p.out_rgb = dev_out_rgb; p.out_alpha = dev_out_alpha; p.out_depth = dev_out_depth; p.out_mask = dev_out_mask;
+    p.out_count = dev_out_count;
+    int n = 0;
+    cudaError_t e = ggt_launch_splat(p, (cudaStream_t)stream, &n);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "splat launch");
+    ctx->launches += n;
+    return GGT_OK;
+}
+
+int ggt_temporal_weight_mask(ggt_ctx* ctx, int64_t n_pixels, const float* dev_prev_depth, const float* dev_prev_conf,
+                             int32_t n_masks, const float* const* dev_masks, float beta, float eta,
+                             float* dev_weight_out, void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    if (!dev_prev_depth || !dev_prev_conf || !dev_masks || !dev_weight_out) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL argument to ggt_temporal_weight_mask");
+    if (n_pixels <= 0) return fail(ctx, GGT_ERR_SHAPE, "n_pixels %lld", (long long)n_pixels);
+    if (n_masks < 1 || n_masks > GGT_MAX_VIEWS) return fail(ctx, GGT_ERR_SHAPE, "n_masks %d not in [1, %d]", n_masks, GGT_MAX_VIEWS);
+    if (!(beta >= 0.0f) || !(eta >= 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "beta and eta must be >= 0");
+    GgtMaskList ml;
+    memset(&ml, 0, sizeof ml);
+    ml.n = n_masks;
+    for (int k = 0; k < n_masks; ++k) {
+        if (!dev_masks[k]) return fail(ctx, GGT_ERR_INVALID_ARG, "dev_masks[%d] is NULL", k);
+        ml.m[k] = dev_masks[k];
+    }
+    cudaError_t e = ggt_launch_temporal_weight_mask((size_t)n_pixels, dev_prev_depth, dev_prev_conf, ml, beta, eta, dev_weight_out,
+                                                    (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "temporal-weight-mask launch");
     ctx->launches += 1;
     return GGT_OK;
 }

@@ -109,6 +109,35 @@ struct GgtWeightParams {    // all views of one ggt_integrate call: one launch, 
     GgtWeightView v[GGT_MAX_VIEWS];
 };
 
+struct GgtSplatParams {     // ggt_splat_forward: one input view's pixel-sized Gaussians into the target
+    int32_t W, H, Wt, Ht;  // source view / target size
+    int32_t rgb_stride;    // bytes per source pixel of rgb (3 or 4)
+    uint32_t capacity;     // list entries the scratch holds
+    float h[9], e[3];      // source pixel / depth -> target homogeneous pixel: (x, y, w) = D * h (uc, vc, 1)^T + e
+    float fx_t, fy_t, cx_t, cy_t, fx_s;
+    float sigma_px, dilation, z_cull;
+    const float* depth;    // source depth, fp32 H x W
+    const uint8_t* rgb;    // source colour (may be null)
+    const float* mask;     // source mask (may be null)
+    float* gauss;          // scratch: 8 floats per source pixel
+    uint32_t* counts;      // scratch: per target pixel
+    uint32_t* pos;         // scratch: per target pixel (list start, then end)
+    uint32_t* block_sums;  // scratch: scan
+    uint32_t* total;       // scratch: 1 word, number of list entries of this call
+    uint32_t* overflow;    // context: max entries ever needed when that exceeded the capacity (0 = never)
+    uint2* entries;        // scratch: {depth bits, source index}
+    float* out_rgb;        // [3][Ht][Wt] (may be null)
+    float* out_alpha;
+    float* out_depth;
+    float* out_mask;
+    int32_t* out_count;
+};
+
+struct GgtMaskList {        // ggt_temporal_weight_mask: the K splatted masks whose channel-wise maximum is M^t
+    int32_t n, pad_;
+    const float* m[GGT_MAX_VIEWS];
+};
+
 struct GgtExtractParams {
     int32_t Wt, Ht, D, n_groups;
     const float* tables;
@@ -129,6 +158,12 @@ struct ggt_ctx {
     bool ws_owned = false;
     uint16_t* cq = nullptr;        // quarter-res block differences of ggt_refine_depth (context-owned)
     size_t cq_bytes = 0;
+    // ggt_splat_forward scratch (context-owned, grown between calls): Gaussian parameters, per-pixel counts / positions,
+    // scan sums, the per-pixel lists; `splat_flags` = {total entries of the last call, overflow high-water mark}
+    void* splat_ws = nullptr;
+    size_t splat_ws_bytes = 0;
+    size_t splat_entries = 0;      // list capacity in entries (0 = automatic: 40 per source pixel)
+    uint32_t* splat_flags = nullptr;
     // ggt_frame_host: host->device copies run on an internal stream so that the next frame's inputs upload while
     // this frame's integrate / extract kernels run.  ev_inputs_free is recorded on the caller's stream once the
     // weight-map pre-pass (the last kernel that reads the uploaded depth / colour buffers) has been enqueued.
@@ -167,6 +202,9 @@ cudaError_t ggt_launch_integrate(const GgtIntegrateParams& p, int dtype, bool fu
 cudaError_t ggt_launch_temporal_weight(const GgtTemporalParams& p, cudaStream_t st);
 cudaError_t ggt_launch_features(const GgtFeatureParams& p, cudaStream_t st);
 cudaError_t ggt_launch_raymarch(const GgtRaymarchParams& p, cudaStream_t st);
+cudaError_t ggt_launch_splat(const GgtSplatParams& p, cudaStream_t st, int* n_launches);
+cudaError_t ggt_launch_temporal_weight_mask(size_t n, const float* prev_depth, const float* prev_conf, const GgtMaskList& masks,
+                                            float beta, float eta, float* out, cudaStream_t st);
 cudaError_t ggt_launch_extract(const GgtExtractParams& p, int dtype, cudaStream_t st);
 cudaError_t ggt_launch_export(const GgtExtractParams& p, int dtype, float* T, float* W, cudaStream_t st);
 cudaError_t ggt_launch_selftest_arith(long long n, const float* a, const float* b, unsigned* mismatch, cudaStream_t st);
