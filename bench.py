@@ -8,8 +8,10 @@ ggt_refine_depth on each of the V views, ggt_integrate (weight maps + fusion), g
   e2e       same metric through ggt_frame_host with pinned HOST buffers (H2D of colour + depth, D2H of
             depth + confidence inside the timed region)
   roofline  dominant kernel (integrate main) timed with CUDA events on its stream via ggt_profile_*
-  cpu_baseline  the oracle as it stands on the host cores, bounded sample
-`--impl reference` times the oracle (tier contract: the reference arm is the oracle).
+  cpu_baseline  the oracle as it stands on one host core: one full step of the same workload
+  extra     (rank 0, default workload only) compact legs for C4 and C5 (a few steps each, roofline fractions recomputed
+            in the run), the fused call, the paper's own raymarch schedule, features, Eq. 3, the Gaussian forward splat
+`--impl reference` times the oracle (tier contract: the reference arm is the oracle): full, unsampled steps.
 """
 import argparse
 import json
@@ -28,6 +30,10 @@ METRIC = "Gvoxel·view TSDF updates/s"
 UNIT = "Gvoxel·view/s"
 REFINE = dict(lambda_t=0.7, beta=0.6, theta=8.0 / 255.0)
 N_INPUT_FRAMES = 3          # distinct synthetic frames cycled through (prev/cur pairs)
+# the roofline time per frame, max(T_bytes at the measured HBM peak, T_fma at peak FP32), as the
+# survey derived it (its bytes assume an interleaved {T, W} volume; this build's planar layout moves fewer)
+SURVEY_T_ROOF_MS = {"C2": 0.037, "C3": 0.66, "C4": 1.00, "C5": 15.9}
+REFERENCE_BUDGET_S = 150.0  # --impl reference: full oracle steps are run while they fit this wall-clock budget
 
 
 def parse_args():
@@ -39,6 +45,7 @@ def parse_args():
     ap.add_argument("--workload", default="C3", choices=["C2", "C3", "C4", "C5"])
     ap.add_argument("--fused", action="store_true", help="use ggt_integrate_extract instead of integrate + extract")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the extra legs (C4 / C5 / raymarch / splat ...)")
     return ap.parse_args()
 
 
@@ -103,22 +110,43 @@ def physical_gpu_index(local_rank):
 # ----------------------------------------------------------------------------------------------------
 # workload set-up (inputs generated on the host by the seeded generator, then made resident in HBM)
 # ----------------------------------------------------------------------------------------------------
+_WL = {}
+
+
+def _gen_view(name, frame, view):
+    """Worker of the input-synthesis pool: one rig view of one frame (depth, colour)."""
+    from paper_2505_18932_b200 import synth
+    if name not in _WL:
+        _WL[name] = synth.workload(name)
+    d, rgb = _WL[name].view_inputs(frame, view)
+    return np.array(d), (None if rgb is None else np.array(rgb))
+
+
+def synth_pool():
+    """Fork pool for the analytic ray-casts (CPU, seconds per 1080p view).  Created before CUDA is initialised."""
+    import multiprocessing as mp
+    world = max(1, int(os.environ.get("WORLD_SIZE", "1")))
+    n = min(12, max(1, ((os.cpu_count() or 2) - 2) // world))
+    return mp.get_context("fork").Pool(n) if n > 1 else None
+
+
 class Inputs:
-    def __init__(self, name, rank, world):
+    def __init__(self, name, rank, world, n_frames=N_INPUT_FRAMES, pool=None):
         from paper_2505_18932_b200 import sharding, synth
         self.wl = wl = synth.workload(name)
-        self.frames = sharding.frames_for_rank(rank, world, N_INPUT_FRAMES)
+        self.n_frames = n_frames
+        self.frames = sharding.frames_for_rank(rank, world, n_frames)
         self.targets = wl.targets(self.frames[0])                  # C5: 8 targets per frame, else 1
         self.vis = [wl.views_for(t) for t in self.targets]
         self.target, self.vi = self.targets[0], self.vis[0]
         self.views = [wl.rig[v] for v in self.vi]
         self.view_ids = sorted(set(v for vi in self.vis for v in vi))     # each rig view is refined once per frame
         self.multi = len(self.targets) > 1
-        if self.multi:
-            self.data_by_view = [{v: wl.view_inputs(f, v) for v in self.view_ids} for f in self.frames]
-            self.data = [[d[v] for v in self.vi] for d in self.data_by_view]
-        else:
-            self.data = [[wl.view_inputs(f, v) for v in self.vi] for f in self.frames]   # [frame][view] -> (depth, rgb)
+        jobs = [(name, f, v) for f in self.frames for v in self.view_ids]
+        res = pool.starmap(_gen_view, jobs) if pool is not None else [_gen_view(*j) for j in jobs]
+        got = dict(zip([(f, v) for _, f, v in jobs], res))
+        self.data_by_view = [{v: got[(f, v)] for v in self.view_ids} for f in self.frames]
+        self.data = [[d[v] for v in self.vi] for d in self.data_by_view]   # [frame][view] -> (depth, rgb)
         self.W, self.H = self.views[0].width, self.views[0].height
         self.V = len(self.vi)
         self.vv_per_step = float(sum(t.width * t.height * wl.z_bins.size * len(vi) for t, vi in zip(self.targets, self.vis)))
@@ -154,14 +182,14 @@ class DeviceRun:
             self.vols.append(vol)
         self.vol = self.vols[0]
         if inp.multi:          # [frame][rig view id] -> tensors; every view of the union is refined once per frame
-            self.depth_by = [{v: torch.from_numpy(np.array(d[v][0])).cuda() for v in inp.view_ids} for d in inp.data_by_view]
-            self.rgb_by = [{v: torch.from_numpy(np.array(d[v][1])).cuda() for v in inp.view_ids} for d in inp.data_by_view]
+            self.depth_by = [{v: torch.from_numpy(d[v][0]).cuda() for v in inp.view_ids} for d in inp.data_by_view]
+            self.rgb_by = [{v: torch.from_numpy(d[v][1]).cuda() for v in inp.view_ids} for d in inp.data_by_view]
             self.state_by = {v: self.depth_by[0][v].clone() for v in inp.view_ids}
             pos = {v: i for i, v in enumerate(inp.view_ids)}
             self.rig_views = [wl.rig[v] for v in inp.view_ids]
             self.view_index = [[pos[v] for v in vi] for vi in inp.vis]
-        self.depth_in = [[torch.from_numpy(np.array(d)).cuda() for d, _ in fr] for fr in inp.data]
-        self.rgb_in = [[torch.from_numpy(np.array(r)).cuda() if r is not None else None for _, r in fr] for fr in inp.data]
+        self.depth_in = [[torch.from_numpy(d).cuda() for d, _ in fr] for fr in inp.data]
+        self.rgb_in = [[torch.from_numpy(r).cuda() if r is not None else None for _, r in fr] for fr in inp.data]
         self.state = [self.depth_in[0][k].clone() for k in range(inp.V)]
         n = inp.target.width * inp.target.height
         self.depth = torch.empty(n, dtype=torch.float32, device="cuda")
@@ -171,7 +199,7 @@ class DeviceRun:
 
     def step(self):
         inp, ctx = self.inp, self.ctx
-        cur = 1 + self.i % (N_INPUT_FRAMES - 1)
+        cur = 1 + self.i % (inp.n_frames - 1)
         prev = cur - 1
         self.i += 1
         if inp.multi:
@@ -204,8 +232,8 @@ class HostRun:
         import torch
         self.torch, self.inp, self.dev = torch, inp, dev
         wl = inp.wl
-        self.rgb = [[torch.from_numpy(np.array(r)).pin_memory() if r is not None else None for _, r in fr] for fr in inp.data]
-        self.dep = [[torch.from_numpy(np.array(d)).pin_memory() for d, _ in fr] for fr in inp.data]
+        self.rgb = [[torch.from_numpy(r).pin_memory() if r is not None else None for _, r in fr] for fr in inp.data]
+        self.dep = [[torch.from_numpy(d).pin_memory() for d, _ in fr] for fr in inp.data]
         n = inp.target.width * inp.target.height
         self.outs = [(torch.empty(n, dtype=torch.float32).pin_memory(), torch.empty(n, dtype=torch.float32).pin_memory())
                      for _ in range(2)]          # two result buffers: the pipelined leg alternates between them
@@ -220,7 +248,7 @@ class HostRun:
 
     def step(self):
         inp, dev = self.inp, self.dev
-        cur = self.i % N_INPUT_FRAMES
+        cur = self.i % inp.n_frames
         self.i += 1
         dev.ctx.ggt_frame_host(dev.vol, inp.target, inp.views, self.rgb[cur] if inp.wl.colour else None, self.dep[cur],
                                list(range(inp.V)), self.slot_state, self.staging, *self.outs[self.i & 1],
@@ -246,13 +274,84 @@ def timed(torch, dist, fn, steps, warmup):
     return e0.elapsed_time(e1)
 
 
+def device_peaks(torch, sampler):
+    """SM count and maximum SM clock read on the box: the FP32 and issue-slot peaks derive from them."""
+    props = torch.cuda.get_device_properties(torch.cuda.current_device())
+    sms = int(props.multi_processor_count)
+    mhz = sampler.max_mhz if sampler is not None and sampler.max_mhz else None
+    src = "NVML max SM clock"
+    if not mhz:
+        mhz = float(getattr(props, "clock_rate", 1965000)) / 1e3
+        src = "cudaDeviceProp.clockRate"
+    hz = float(mhz) * 1e6
+    return {"sm_count": sms, "sm_max_mhz": float(mhz), "clock_source": src,
+            "fp32_tflops": sms * 128 * 2 * hz / 1e12, "issue_per_s": sms * 4 * hz}
+
+
+def stage_profile(torch, dev, steps):
+    """Per-stage device time of `steps` steps (events around each kernel group on the launching stream)."""
+    dev.ctx.ggt_profile_enable(True)
+    torch.cuda.synchronize()
+    for _ in range(steps):
+        dev.step()
+    torch.cuda.synchronize()
+    prof = dev.ctx.ggt_profile_collect()
+    dev.ctx.ggt_profile_enable(False)
+    return prof, {k: (v[0] / max(steps, 1)) for k, v in prof.items()}
+
+
+def roofline_of(inp, prof, stage_ms, fused, hbm_peak, peak_src, peaks):
+    """Roofline object of the dominant kernel (k_integrate) plus the north_star quantity integrate + extract."""
+    t, wl = inp.target, inp.wl
+    voxels = t.width * t.height * wl.z_bins.size
+    vox_bytes = voxels * (4 if wl.storage == "f16" else 8)
+    map_bytes = inp.V * inp.W * inp.H * 8
+    integ_bytes = vox_bytes * (2 if wl.persistent else 1) + map_bytes      # algorithmic: DESIGN.md "Roofline"
+    integ_ms = prof["integrate"][0] / max(prof["integrate"][1], 1)
+    achieved = integ_bytes / (integ_ms / 1e3) / 1e9 if integ_ms > 0 else 0.0
+    nt = len(inp.targets)
+    # extract searches the T plane only (half of the volume) and fetches W for the crossing candidates
+    path_bytes = (integ_bytes + (0 if fused else vox_bytes // 2) + 2 * t.width * t.height * 4) * nt
+    path_ms = stage_ms["integrate"] + stage_ms["extract"]
+    vv = inp.vv_per_step
+    flops = 16.0 * vv + 12.0 * voxels * nt                               # SURVEY.md 8(d): 16 per voxel.view + 8 + 4 per voxel
+    t_bytes_ms = path_bytes / (hbm_peak * 1e9) * 1e3
+    t_fma_ms = flops / (peaks["fp32_tflops"] * 1e12) * 1e3
+    t_roof = max(t_bytes_ms, t_fma_ms)
+    s_roof = SURVEY_T_ROOF_MS.get(wl.name)
+    roof = {"bound": "hbm", "kernel": "k_integrate (ggt_integrate main kernel)", "achieved": achieved, "peak": hbm_peak,
+            "unit": "GB/s", "frac": achieved / hbm_peak, "traffic": None, "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": integ_bytes, "ms_per_launch": integ_ms,
+            "integrate_plus_extract": {"bytes": path_bytes, "ms": path_ms,
+                                       "frac": (path_bytes / (path_ms / 1e3) / 1e9 / hbm_peak) if path_ms > 0 else 0.0,
+                                       "t_bytes_ms": t_bytes_ms, "t_fma_ms": t_fma_ms,
+                                       "frac_of_max_tbytes_tfma": t_roof / path_ms if path_ms > 0 else 0.0,
+                                       "survey_t_roof_ms": s_roof,
+                                       "frac_of_survey_t_roof": (s_roof / path_ms) if path_ms > 0 and s_roof else None},
+            "alu": {"flop_per_voxel_view": 16, "achieved_tflops": 16 * vv / nt / (integ_ms / 1e3) / 1e12 if integ_ms > 0 else 0.0,
+                    "peak_tflops_at_max_clock": peaks["fp32_tflops"], "sm_count": peaks["sm_count"],
+                    "sm_max_mhz": peaks["sm_max_mhz"], "clock_source": peaks["clock_source"]}}
+    traffic_file = os.path.join(ROOT, "profiles", "traffic_integrate.json")
+    if os.path.exists(traffic_file):
+        with open(traffic_file) as fh:
+            tj = json.load(fh)
+        roof["traffic"] = tj.get(wl.name + ("_fused" if fused else ""))
+        roof["traffic_source"] = "profiles/traffic_integrate.json (ncu --set full capture of this kernel; not measured in this run)"
+        wi = tj.get(wl.name + "_warp_instructions")
+        if wi and not fused and integ_ms > 0:
+            # the kernel's practical limit: one warp instruction per SM sub-partition per clock; the instruction count is
+            # the ncu-measured one of the committed profile (static for this workload)
+            roof["issue"] = {"warp_instructions_per_launch": wi, "peak_warp_instructions_per_s": peaks["issue_per_s"],
+                             "frac": wi / peaks["issue_per_s"] / (integ_ms / 1e3)}
+    return roof, integ_ms
+
+
 # ----------------------------------------------------------------------------------------------------
 # the oracle, timed as it stands on the host cores (cpu_baseline leg and --impl reference)
 # ----------------------------------------------------------------------------------------------------
-def oracle_step(inp, ray_every, cur=1):
-    """One step of the whole path on the CPU oracle: refine + weight maps in full for the V views,
-    integrate + extract on a seeded 1/ray_every subset of the target rays.  Returns the wall time
-    extrapolated to the full frame (ray-dependent part scaled by the sampling ratio) and its parts."""
+def oracle_step(inp, cur=1, ray_every=1):
+    """One step of the whole path on the CPU oracle, single-threaded: refine + weight maps of the V views, integrate +
+    extract of the target (every ray when ray_every = 1).  Returns the wall time and its parts."""
     import oracle
     wl, tgt = inp.wl, inp.target
     t0 = time.perf_counter()
@@ -267,55 +366,128 @@ def oracle_step(inp, ray_every, cur=1):
     maps = [oracle.weight_map(d) for d in depths]
     t2 = time.perf_counter()
     n = tgt.width * tgt.height
-    rays = np.arange(ray_every // 2, n, ray_every, dtype=np.int32)
+    rays = None if ray_every <= 1 else np.arange(ray_every // 2, n, ray_every, dtype=np.int32)
     tau = oracle.tau_table(wl.z_bins, wl.trunc_bins)
     T, W = oracle.integrate(tgt, wl.z_bins, tau, inp.views, maps, rays=rays, accumulate=wl.persistent,
                             cap=wl.weight_cap, half_storage=wl.storage == "f16")
     oracle.extract(wl.z_bins, T, W)
     t3 = time.perf_counter()
-    scale = n / float(rays.size)
-    full = (t1 - t0) + (t2 - t1) + (t3 - t2) * scale
-    return full, {"refine_s": t1 - t0, "weight_s": t2 - t1, "integrate_extract_sample_s": t3 - t2,
-                  "rays": int(rays.size), "measured_s": t3 - t0}
+    return t3 - t0, {"refine_s": t1 - t0, "weight_s": t2 - t1, "integrate_extract_s": t3 - t2,
+                     "rays": n if rays is None else int(rays.size)}
 
 
-def cpu_baseline(inp, ray_every=2):
-    full, parts = oracle_step(inp, ray_every)
+def cpu_baseline(inp):
+    full, parts = oracle_step(inp)
     return {"value": inp.vv_per_step / full / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": "one %s step: refine + weight maps of all %d views in full, integrate + extract on every %d-th "
-                      "target ray (%d rays), ray part scaled by the sampling ratio; %.1f s of CPU work, "
-                      "extrapolated %.1f s per frame; host has %d cores, the oracle is single-threaded"
-                      % (inp.wl.name, inp.V, ray_every, parts["rays"], parts["measured_s"], full, os.cpu_count() or 0),
-            "ms_per_step_extrapolated": full * 1e3}
+            "sample": "one full %s step, nothing sampled or extrapolated: refine + weight maps of all %d views, integrate + extract "
+                      "of all %d target rays; %.1f s of CPU work (refine %.1f, weight maps %.1f, integrate + extract %.1f); host has "
+                      "%d cores, the oracle is single-threaded"
+                      % (inp.wl.name, inp.V, parts["rays"], full, parts["refine_s"], parts["weight_s"], parts["integrate_extract_s"],
+                         os.cpu_count() or 0),
+            "ms_per_step": full * 1e3}
 
 
 def run_reference(args, rank, world):
-    """--impl reference: the oracle on the host cores (rank 0 only), same metric / config."""
+    """--impl reference: the oracle on the host cores (rank 0 only), same metric / config; every timed step is a full,
+    unsampled step; as many of the requested steps as fit REFERENCE_BUDGET_S are run."""
     if rank != 0:
         return
-    inp = Inputs(args.workload, 0, 1)
-    ray_every = 64
-    for _ in range(min(args.warmup, 1)):
-        oracle_step(inp, ray_every)
-    fulls, parts = [], None
-    steps = max(1, min(args.steps, 5))           # bounded: each sampled step is ~6 s of CPU work
-    for i in range(steps):
-        full, parts = oracle_step(inp, ray_every, cur=1 + i % (N_INPUT_FRAMES - 1))
-        fulls.append(full)
-    ms = float(np.mean(fulls)) * 1e3
+    t_start = time.perf_counter()
+    pool = synth_pool()
+    inp = Inputs(args.workload, 0, 1, pool=pool)
+    if pool is not None:
+        pool.close()
+    if inp.multi:
+        print(json.dumps({"impl": "reference", "unavailable": "the oracle leg runs the single-target workloads (C2-C4)"}))
+        return
+    warm = min(args.warmup, 1)
+    for _ in range(warm):
+        oracle_step(inp, ray_every=64)           # pages the library and the inputs in; not timed
+    times, parts = [], None
+    while len(times) < max(1, args.steps):
+        if times and (time.perf_counter() - t_start) + 1.1 * max(times) > REFERENCE_BUDGET_S:
+            break
+        dt, parts = oracle_step(inp, cur=1 + len(times) % (inp.n_frames - 1))
+        times.append(dt)
+    ms = float(np.mean(times)) * 1e3
     value = inp.vv_per_step / (ms / 1e3) / 1e9
-    sample = ("each step: refine + weight maps of all %d views in full, integrate + extract on every %dth ray (%d rays), "
-              "extrapolated to the frame; %d of the requested %d steps run (bounded)" % (inp.V, ray_every, parts["rays"], steps, args.steps))
-    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
-            "warmup": min(args.warmup, 1), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": inp.describe(1),
+    sample = ("each step: one full %s step of the oracle, single-threaded, nothing sampled or extrapolated (refine + weight maps of "
+              "all %d views, integrate + extract of all %d rays); %d of the requested %d steps run within the %.0f s budget"
+              % (inp.wl.name, inp.V, parts["rays"], len(times), args.steps, REFERENCE_BUDGET_S))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": len(times),
+            "steps_requested": args.steps, "steps_run": len(times), "warmup": warm, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": inp.describe(1),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gpu_launches": 0}
+            "gpu_launches": 0, "wall_s": time.perf_counter() - t_start}
     print(json.dumps(line))
 
 
 # ----------------------------------------------------------------------------------------------------
+def fused_batch_frame(dev, d8, c8):
+    inp, ids = dev.inp, dev.inp.view_ids
+    dev.ctx.ggt_refine_depth_batch([dev.rgb_by[1][v] for v in ids], [dev.rgb_by[0][v] for v in ids],
+                                   [dev.depth_by[1][v] for v in ids], [dev.state_by[v] for v in ids], **REFINE)
+    dev.ctx.ggt_integrate_extract_batch(dev.vols, inp.targets, dev.rig_views, [dev.state_by[v] for v in ids],
+                                        dev.view_index, dev.flags, depth=d8, conf=c8)
+
+
+def compact_leg(torch, name, pool, hbm_peak, peak_src, peaks, steps, warmup):
+    """extra.C4 / extra.C5: a few steps of another BASELINE.json config with its roofline fractions recomputed in the run."""
+    inp = Inputs(name, 0, 1, n_frames=2, pool=pool)
+    dev = DeviceRun(inp, False)
+    for _ in range(warmup):
+        dev.step()
+    launches0 = dev.ctx.launch_count
+    ms = timed(torch, None, dev.step, steps, 0) / steps
+    launches = (dev.ctx.launch_count - launches0) // steps
+    prof, stage_ms = stage_profile(torch, dev, steps)
+    roof, integ_ms = roofline_of(inp, prof, stage_ms, False, hbm_peak, peak_src, peaks)
+    out = {"config": inp.describe(1)["workload"], "steps": steps, "warmup": warmup, "ms_per_step": ms,
+           "ms_per_target": ms / len(inp.targets), "gvoxel_view_per_s": inp.vv_per_step / (ms / 1e3) / 1e9,
+           "stages_ms": {"refine_all_views": stage_ms["refine"], "weight_maps": stage_ms["weight"],
+                         "integrate": stage_ms["integrate"], "extract": stage_ms["extract"]},
+           "k_integrate_ms_per_launch": integ_ms, "gpu_launches_per_step": int(launches), "roofline": roof}
+    if inp.multi:
+        d8 = [torch.empty_like(dev.depth) for _ in inp.targets]
+        c8 = [torch.empty_like(dev.conf) for _ in inp.targets]
+        out["fused_batch_frame_ms"] = timed(torch, None, lambda: fused_batch_frame(dev, d8, c8), steps, 1) / steps
+    else:
+        depths = dev.depth_in[1]
+        fused_fn = lambda: dev.ctx.ggt_integrate_extract(dev.vol, inp.target, inp.views, depths, dev.flags, dev.depth, dev.conf)
+        out["fused_integrate_extract_ms"] = timed(torch, None, fused_fn, steps, 1) / steps
+    del dev
+    torch.cuda.empty_cache()
+    return out
+
+
+def splat_leg(torch, binding, wl, k):
+    """f-3 at PAPER.md Table 4's shape: K = 4 views of 1352x1014 forward-splatted into a 1352x1014 target."""
+    from paper_2505_18932_b200 import synth
+    rig = synth.grid_rig(1352, 1014)
+    tgt = rig[5]
+    vi = synth.nearest_views(tgt, rig, 4, exclude=5)
+    ctx = binding.Context()
+    ins = []
+    for i in vi:
+        d, rgb = synth.raycast(rig[i], wl.scene, 0.0, want_colour=True)
+        ins.append((rig[i], torch.from_numpy(synth.noisy_depth(d, 1352, i, 0.01, 0.02)).cuda(), torch.from_numpy(rgb).cuda(),
+                    torch.full(d.shape, 0.7, dtype=torch.float32, device="cuda")))
+    n = 1352 * 1014
+    outs = [(torch.empty((3, 1014, 1352), device="cuda"), torch.empty(n, device="cuda"), torch.empty(n, device="cuda"),
+             torch.empty(n, device="cuda")) for _ in vi]
+
+    def fn():
+        for (cam, d, rgb, m), (o_rgb, o_a, o_d, o_m) in zip(ins, outs):
+            ctx.ggt_splat_forward(tgt, cam, d, rgb=rgb, mask=m, out_rgb=o_rgb, out_alpha=o_a, out_depth=o_d, out_mask=o_m)
+    ms = timed(torch, None, fn, k, 2) / k
+    last, need = ctx.ggt_splat_status()
+    return {"call": "ggt_splat_forward x 4 views (PAPER.md:63-67, 362-368): K = 4 views of 1352x1014 into a 1352x1014 target, colour + "
+                    "opacity + depth + mask each (the resolution of PAPER.md Table 4's 10 ms forward-splatting stage, GPU not stated)",
+            "ms_per_frame_4_views": ms, "ms_per_view": ms / 4, "list_entries_last_view": last, "overflow": need,
+            "coverage_last_view": float((outs[-1][1] > 0.5).float().mean().item()), "paper_ms": 10.0}
+
+
 def main():
     args = parse_args()
     from paper_2505_18932_b200 import sharding
@@ -323,6 +495,9 @@ def main():
     if args.impl == "reference":
         run_reference(args, rank, world)
         return
+    # input synthesis (CPU ray-casts) in a fork pool, before CUDA is initialised in this process
+    pool = synth_pool()
+    inp = Inputs(args.workload, rank, world, pool=pool)
     import torch
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
@@ -340,14 +515,13 @@ def main():
     if dist is not None:
         dist.barrier()
 
-    inp = Inputs(args.workload, rank, world)
     dev = DeviceRun(inp, args.fused)
     host = HostRun(inp, dev) if not inp.multi else None
     hbm_peak, peak_src, _ = measured_peaks()
 
     # ---- headline: device-resident inputs --------------------------------------------------------------
     sampler = ClockSampler(physical_gpu_index(local_rank))
-    launches0 = dev.ctx.launch_count
+    peaks = device_peaks(torch, sampler)
     for _ in range(args.warmup):
         dev.step()
     launches_w = dev.ctx.launch_count
@@ -361,43 +535,9 @@ def main():
     value = red["units"] / (red["ms"] / 1e3) / 1e9
 
     # ---- per-stage device time of the same step (events around each kernel group, same stream) ---------
-    dev.ctx.ggt_profile_enable(True)
-    torch.cuda.synchronize()
-    for _ in range(args.steps):
-        dev.step()
-    torch.cuda.synchronize()
-    prof = dev.ctx.ggt_profile_collect()
-    dev.ctx.ggt_profile_enable(False)
-    stage_ms = {k: (v[0] / max(args.steps, 1)) for k, v in prof.items()}
+    prof, stage_ms = stage_profile(torch, dev, args.steps)
+    roofline, integ_ms = roofline_of(inp, prof, stage_ms, args.fused, hbm_peak, peak_src, peaks)
     t, wl = inp.target, inp.wl
-    voxels = t.width * t.height * wl.z_bins.size
-    vox_bytes = voxels * (4 if wl.storage == "f16" else 8)
-    map_bytes = inp.V * inp.W * inp.H * 8
-    integ_bytes = vox_bytes * (2 if wl.persistent else 1) + map_bytes      # algorithmic: DESIGN.md "Roofline"
-    integ_ms = prof["integrate"][0] / max(prof["integrate"][1], 1)
-    achieved = integ_bytes / (integ_ms / 1e3) / 1e9 if integ_ms > 0 else 0.0
-    # extract searches the T plane only (half of the volume) and fetches W for the crossing candidates
-    path_bytes = (integ_bytes + (0 if args.fused else vox_bytes // 2) + 2 * t.width * t.height * 4) * len(inp.targets)
-    path_ms = stage_ms["integrate"] + stage_ms["extract"]
-    roofline = {"bound": "hbm", "kernel": "k_integrate (ggt_integrate main kernel)", "achieved": achieved, "peak": hbm_peak,
-                "unit": "GB/s", "frac": achieved / hbm_peak, "traffic": None, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": integ_bytes, "ms_per_launch": integ_ms,
-                "integrate_plus_extract": {"bytes": path_bytes, "ms": path_ms,
-                                           "frac": (path_bytes / (path_ms / 1e3) / 1e9 / hbm_peak) if path_ms > 0 else 0.0},
-                "alu": {"flop_per_voxel_view": 16, "achieved_tflops": 16 * inp.vv_per_step / len(inp.targets) / (integ_ms / 1e3) / 1e12 if integ_ms > 0 else 0.0,
-                        "peak_tflops_at_max_clock": 148 * 128 * 2 * 1.965e9 / 1e12}}
-    traffic_file = os.path.join(ROOT, "profiles", "traffic_integrate.json")
-    if os.path.exists(traffic_file):
-        with open(traffic_file) as fh:
-            tj = json.load(fh)
-        roofline["traffic"] = tj.get(wl.name + ("_fused" if args.fused else ""))
-        wi = tj.get(wl.name + "_warp_instructions")
-        if wi and not args.fused and integ_ms > 0:
-            # the kernel's practical limit: one warp instruction per SM sub-partition per clock (148 SMs x 4 x 1.965 GHz);
-            # the instruction count is the ncu-measured one of the committed profile (static for this workload)
-            peak_issue = 148 * 4 * 1.965e9
-            roofline["issue"] = {"warp_instructions_per_launch": wi, "peak_warp_instructions_per_s": peak_issue,
-                                 "frac": wi / peak_issue / (integ_ms / 1e3)}
 
     # ---- e2e: host buffers through ggt_frame_host, result needed on the host every step ----------------
     if inp.multi:
@@ -419,26 +559,19 @@ def main():
         e2e["pipelined"] = {"value": red_p["units"] / (red_p["ms"] / 1e3) / 1e9, "unit": UNIT, "ms_per_step": red_p["ms"] / e2e_steps,
                             "note": "same per-step copies, no host synchronise between steps (throughput of an online stream)"}
 
+    extra = {}
+    do_extra = rank == 0 and not args.no_extra
     # ---- C5 only: the same frame with the zero-crossing search fused into the batch (no volume re-read) ---------
-    extra_multi = {}
-    if rank == 0 and inp.multi:
-        ids = inp.view_ids
+    if do_extra and inp.multi:
         d8 = [torch.empty_like(dev.depth) for _ in inp.targets]
         c8 = [torch.empty_like(dev.conf) for _ in inp.targets]
-
-        def fused_frame():
-            dev.ctx.ggt_refine_depth_batch([dev.rgb_by[1][v] for v in ids], [dev.rgb_by[0][v] for v in ids],
-                                           [dev.depth_by[1][v] for v in ids], [dev.state_by[v] for v in ids], **REFINE)
-            dev.ctx.ggt_integrate_extract_batch(dev.vols, inp.targets, dev.rig_views, [dev.state_by[v] for v in ids],
-                                                dev.view_index, dev.flags, depth=d8, conf=c8)
         kf = max(3, min(args.steps, 10))
-        ms_ff = timed(torch, None, fused_frame, kf, 2) / kf
-        extra_multi["fused_batch_frame"] = {"call": "ggt_refine_depth_batch + ggt_integrate_extract_batch (8 targets, no volume re-read)",
-                                            "ms_per_frame": ms_ff}
+        ms_ff = timed(torch, None, lambda: fused_batch_frame(dev, d8, c8), kf, 2) / kf
+        extra["fused_batch_frame"] = {"call": "ggt_refine_depth_batch + ggt_integrate_extract_batch (8 targets, no volume re-read)",
+                                      "ms_per_frame": ms_ff}
 
     # ---- extra legs (not the headline): fused integrate+extract, and the paper's own volume-free schedule ------
-    extra = {}
-    if rank == 0 and not inp.multi:
+    if do_extra and not inp.multi:
         k = max(3, min(args.steps, 20))
         depths = dev.state if wl.colour else dev.depth_in[1]
         fused_fn = lambda: dev.ctx.ggt_integrate_extract(dev.vol, inp.target, inp.views, depths, dev.flags, dev.depth, dev.conf)
@@ -489,6 +622,7 @@ def main():
         ft_bytes = n_t * (4 + 16 * inp.V)
         extra["guidance_features"] = {"call": "ggt_guidance_features (PAPER.md:374-388 items 5-8), [4K][H][W] fp32", "ms_per_call": ms_ft,
                                       "algorithmic_bytes": ft_bytes, "frac_of_hbm_peak": ft_bytes / (ms_ft / 1e3) / 1e9 / hbm_peak}
+        del feats
         # Eq. 3 (f-2): the previous output depth as a (V+1)-th view with Eq. 13's weight, masks from ggt_refine_depth
         Hv, Wv = inp.H, inp.W
         masks = [torch.full((Hv, Wv), 0.6, dtype=torch.float32, device="cuda") for _ in range(inp.V)]
@@ -508,6 +642,22 @@ def main():
             "call": "ggt_temporal_weight (Eq. 13-14) + ggt_raymarch_depth_weighted with D^{t-1} as view V+1 (Eq. 3)",
             "temporal_weight_ms": ms_tw, "raymarch_weighted_ms_per_call": ms_r5, "views": inp.V + 1,
             "evaluations_per_ray_mean": float(steps_out.sum().item()) / n_t}
+        del masks, prev_d, prev_c, wmap
+        # f-3: the Gaussian forward splat at Table 4's shape
+        extra["gaussian_forward_splat"] = splat_leg(torch, dev.b, wl, max(3, min(args.steps, 10)))
+
+    # ---- the other 1080p / batched configs, a few steps each (default workload, one GPU) -------------------------
+    if do_extra and world == 1 and args.workload == "C3":
+        host = None
+        dev.vols, dev.vol = [], None           # release the C3 volume before the 34 GB of C5
+        torch.cuda.empty_cache()
+        for name, ks in (("C4", 5), ("C5", 3)):
+            try:
+                extra[name] = compact_leg(torch, name, pool, hbm_peak, peak_src, peaks, ks, 3)
+            except Exception as exc:           # a leg that cannot run (e.g. memory) is reported, never silently dropped
+                extra[name] = {"error": repr(exc)}
+    if pool is not None:
+        pool.close()
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -521,8 +671,8 @@ def main():
                 "ms_per_1080p_target_frame": ms_per_step,
                 "integrate_gvoxel_view_per_s": inp.vv_per_step / len(inp.targets) / (integ_ms / 1e3) / 1e9 if integ_ms > 0 else None,
                 "ms_per_target": ms_per_step / len(inp.targets),
-                "paper_context": "PAPER.md Table 4: TSDF stage 6 ms/frame at 1352x1014, K=4, GPU not stated",
-                "extra": extra if not inp.multi else extra_multi}
+                "paper_context": "PAPER.md Table 4: TSDF stage 6 ms/frame, forward splatting 10 ms at 1352x1014, K=4, GPU not stated",
+                "extra": extra}
         if not args.no_cpu_baseline and world == 1 and not inp.multi:
             line["cpu_baseline"] = cpu_baseline(inp)
         print(json.dumps(line))

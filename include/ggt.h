@@ -119,7 +119,9 @@ int ggt_set_workspace(ggt_ctx* ctx, void* dev_workspace, size_t bytes);
 /* ---- volume ------------------------------------------------------------------------------------- */
 /* Bytes the caller must allocate for a volume: a 256-B-aligned table header (z_j, tau_j) followed by
  * the voxels in the internal layout  T[ceil(D/G)][H_t][W_t][G]  then  W[ceil(D/G)][H_t][W_t][G]  with G = 4 (fp32)
- * or 8 (fp16) bins per 128-bit access; bins are padded to a multiple of G. */
+ * or 8 (fp16) bins per 128-bit access (bins are padded to a multiple of G), followed by one
+ * 16-bit search hint per target ray (written by ggt_integrate*, read by ggt_extract_depth: the first group of bins
+ * that holds a non-positive T).  The storage is opaque: only the ggt_* calls may write it. */
 size_t ggt_volume_bytes(const ggt_volume_desc* desc);
 /* Binds caller-owned device storage (>= ggt_volume_bytes, 256-B aligned) and uploads the bin tables
  * (synchronous small copy).  The storage content is otherwise untouched: call ggt_volume_reset. */

@@ -94,8 +94,10 @@ size_t header_bytes_of(const ggt_volume_desc* d) {
 size_t voxel_bytes_of(const ggt_volume_desc* d) {
     const int G = ggt_group_of(d->dtype);
     const int ng = (d->bins + G - 1) / G;
-    return (size_t)ng * d->width * d->height * 32;     // one 128-bit word per group and pixel in each of the two planes
+    return align_up((size_t)ng * d->width * d->height * 32, 256);     // one 128-bit word per group and pixel in each of the two planes
 }
+
+size_t hint_bytes_of(const ggt_volume_desc* d) { return align_up((size_t)d->width * d->height * sizeof(uint16_t), 256); }
 
 }  // namespace
 
@@ -192,7 +194,7 @@ int ggt_set_workspace(ggt_ctx* ctx, void* dev_workspace, size_t bytes) {
 
 size_t ggt_volume_bytes(const ggt_volume_desc* desc) {
     if (!desc || desc->width <= 0 || desc->height <= 0 || desc->bins < 2) return 0;
-    return header_bytes_of(desc) + voxel_bytes_of(desc);
+    return header_bytes_of(desc) + voxel_bytes_of(desc) + hint_bytes_of(desc);
 }
 
 int ggt_volume_bind(ggt_ctx* ctx, const ggt_volume_desc* desc, void* dev_storage, size_t bytes, ggt_volume** out) {
@@ -229,6 +231,8 @@ int ggt_volume_bind(ggt_ctx* ctx, const ggt_volume_desc* desc, void* dev_storage
     v->voxel_bytes = voxel_bytes_of(desc);
     v->dev_tables = static_cast<float*>(dev_storage);
     v->dev_voxels = static_cast<char*>(dev_storage) + v->header_bytes;
+    v->hint_bytes = hint_bytes_of(desc);
+    v->dev_hints = reinterpret_cast<uint16_t*>(static_cast<char*>(dev_storage) + v->header_bytes + v->voxel_bytes);
     const int Dpad = v->n_groups * v->group;
     std::vector<float> tab(2 * (size_t)Dpad);
     for (int j = 0; j < Dpad; ++j) {
@@ -250,7 +254,8 @@ int ggt_volume_unbind(ggt_ctx*, ggt_volume* vol) {
 
 int ggt_volume_reset(ggt_ctx* ctx, ggt_volume* vol, void* stream) {
     if (!ctx || !vol) return GGT_ERR_INVALID_ARG;
-    cudaError_t e = cudaMemsetAsync(vol->dev_voxels, 0, vol->voxel_bytes, (cudaStream_t)stream);
+    // voxels and, right behind them, the per-ray search hints (0 = search everything)
+    cudaError_t e = cudaMemsetAsync(vol->dev_voxels, 0, vol->voxel_bytes + vol->hint_bytes, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "volume reset");
     ctx->launches += 1;
     return GGT_OK;
@@ -259,7 +264,7 @@ int ggt_volume_reset(ggt_ctx* ctx, ggt_volume* vol, void* stream) {
 static GgtExtractParams extract_params(const ggt_volume* vol) {
     GgtExtractParams p;
     p.Wt = vol->desc.width; p.Ht = vol->desc.height; p.D = vol->desc.bins; p.n_groups = vol->n_groups;
-    p.tables = vol->dev_tables; p.voxels = vol->dev_voxels;
+    p.tables = vol->dev_tables; p.voxels = vol->dev_voxels; p.hint = vol->dev_hints;
     p.depth = nullptr; p.conf = nullptr; p.bin = nullptr;
     return p;
 }
@@ -443,7 +448,7 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
     p.plane = (unsigned long long)vol->desc.width * (unsigned long long)vol->desc.height;
     p.accumulate = flags == GGT_ACCUMULATE ? 1 : 0;
     p.decay = vol->desc.decay; p.cap = vol->desc.weight_cap;
-    p.tables = vol->dev_tables; p.voxels = vol->dev_voxels;
+    p.tables = vol->dev_tables; p.voxels = vol->dev_voxels; p.hint = vol->dev_hints;
     p.depth = dev_depth; p.conf = dev_conf; p.bin = dev_bin;
     {
         const int rc = prepare_views(ctx, target, n_views, views, dev_depths, dev_weights, vol->desc.w_sigma0, vol->desc.w_clip,
@@ -452,7 +457,7 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
     }
     StageTimer tm(ctx, GGT_STAGE_INTEGRATE, st);
     detect_fast_paths(p, n_views);
-    cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, fused, st);
+    cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, fused, ctx->sm_count, st);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "integrate launch");
     ctx->launches += 1;
     return GGT_OK;
@@ -513,7 +518,7 @@ static int integrate_batch_impl(ggt_ctx* ctx, int32_t n_targets, ggt_volume* con
         p.plane = (unsigned long long)vol->desc.width * (unsigned long long)vol->desc.height;
         p.accumulate = flags == GGT_ACCUMULATE ? 1 : 0;
         p.decay = vol->desc.decay; p.cap = vol->desc.weight_cap;
-        p.tables = vol->dev_tables; p.voxels = vol->dev_voxels;
+        p.tables = vol->dev_tables; p.voxels = vol->dev_voxels; p.hint = vol->dev_hints;
         if (fused) {
             p.depth = dev_depth_out ? dev_depth_out[t] : nullptr;
             p.conf = dev_conf_out ? dev_conf_out[t] : nullptr;
@@ -525,7 +530,7 @@ static int integrate_batch_impl(ggt_ctx* ctx, int32_t n_targets, ggt_volume* con
         }
         detect_fast_paths(p, n_views);
         StageTimer tm(ctx, GGT_STAGE_INTEGRATE, st);
-        cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, fused, st);
+        cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, fused, ctx->sm_count, st);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "integrate launch");
         ctx->launches += 1;
     }

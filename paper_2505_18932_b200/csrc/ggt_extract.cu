@@ -4,17 +4,11 @@
 //
 // One thread per target ray.  The volume is two planes per group, [group][v][u] x {G values of T} and the same for
 // W (G = 4 bins fp32, 8 bins fp16): the search reads the T plane only (128-bit words, 512 contiguous bytes per warp
-// request), UNROLL groups ahead,
+// request), UNROLL groups ahead, starting at the per-ray hint k_integrate left (the first group with a bin T <= 0),
 // and fetches weights just for the candidates; after each batch a warp vote (__all_sync) ends the march for the warp
-// once all 32 rays have their crossing, so the kernel reads at most half of the volume, up to the front-most surface.
+// once all 32 rays have their crossing: a warp reads the groups between its front-most hint and its last crossing.
 #include "ggt_internal.h"
 
-#ifndef GGT_EXTRACT_UNROLL_F32
-#define GGT_EXTRACT_UNROLL_F32 8
-#endif
-#ifndef GGT_EXTRACT_UNROLL_F16
-#define GGT_EXTRACT_UNROLL_F16 4
-#endif
 
 namespace {
 
@@ -49,7 +43,7 @@ template <bool HALF>
 __global__ void __launch_bounds__(256)
 k_extract(const __grid_constant__ GgtExtractParams p) {
     constexpr int G = HALF ? 8 : 4;
-    constexpr int UNROLL = HALF ? GGT_EXTRACT_UNROLL_F16 : GGT_EXTRACT_UNROLL_F32;   // 128-bit loads in flight per thread
+    constexpr int UNROLL = HALF ? 2 : 4;                 // 128-bit loads in flight per thread: 16 bins per batch
     extern __shared__ float s_z[];                       // z[Dpad]
     const int Dpad = p.n_groups * G;
     for (int i = threadIdx.y * 32 + threadIdx.x; i < Dpad; i += 256) s_z[i] = __ldg(p.tables + i);
@@ -65,7 +59,12 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
     // The search runs on the T plane alone (half of the volume's bytes): a candidate is T_{j-1} > 0 >= T_j; only then
     // are the two weights fetched, and the candidate is a crossing if both bins were observed (reading P13).  An
     // unobserved bin holds T = 0, so it ends a positive run as a candidate and is then rejected by its W = 0.
-    bool found = !live;
+    // k_integrate left, per ray, the first group that holds a bin with T <= 0 (n_groups: none; 0 after a reset).  The
+    // far bin of a crossing is such a bin, so the search starts one group before the hint: the front-most hint of the
+    // warp's 32 rays, to keep its loads coalesced.  A ray without such a bin has no crossing.
+    const int my_hint = live ? (int)__ldg(p.hint + ((size_t)v * p.Wt + u)) : p.n_groups;
+    const int g_start = max((int)__reduce_min_sync(0xffffffffu, (unsigned)my_hint) - 1, 0) / UNROLL * UNROLL;
+    bool found = !live || my_hint >= p.n_groups;
     float pT = 0.0f;
     float out_d = 0.0f, out_c = 0.0f;
     int out_b = -1;
@@ -91,7 +90,7 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
         }
     };
     uint32_t ppos = 0, plast = 0;                        // fp16: "> 0" mask and raw bits of the previous half2
-    for (int g = 0; g < p.n_groups; g += UNROLL) {
+    for (int g = g_start; g < p.n_groups; g += UNROLL) {
         uint4 w[UNROLL];
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q)

@@ -30,7 +30,8 @@ struct GgtIntegrateParams {
     float decay, cap;
     unsigned long long plane;   // Wt * Ht: 128-bit words per group of the volume
     const float* tables;   // device: z[0..Dpad) then tau[0..Dpad), Dpad = n_groups * G
-    void* voxels;          // device: [n_groups][Ht][Wt][G][{T,W}]
+    void* voxels;          // device: T[n_groups][Ht][Wt][G] then W[n_groups][Ht][Wt][G]
+    uint16_t* hint;        // device: per ray, first group holding a bin with T <= 0 (n_groups = none): ggt_extract_depth's start
     float* depth;          // fused extract outputs (may be null)
     float* conf;
     int32_t* bin;
@@ -142,6 +143,7 @@ struct GgtExtractParams {
     int32_t Wt, Ht, D, n_groups;
     const float* tables;
     const void* voxels;
+    const uint16_t* hint;  // per ray search hint written by k_integrate (0 after a reset: search everything)
     float* depth;
     float* conf;
     int32_t* bin;
@@ -189,6 +191,8 @@ struct ggt_volume {
     size_t voxel_bytes = 0;
     float* dev_tables = nullptr;   // inside the caller's storage
     void* dev_voxels = nullptr;    // inside the caller's storage
+    uint16_t* dev_hints = nullptr; // inside the caller's storage, after the voxels: one search hint per ray
+    size_t hint_bytes = 0;
 };
 
 static inline int ggt_group_of(int dtype) { return dtype == GGT_F16 ? 8 : 4; }
@@ -198,7 +202,7 @@ cudaError_t ggt_launch_refine(int W, int H, const GgtRefineViews& tab, int strid
                               cudaStream_t st, int* n_launches);
 cudaError_t ggt_launch_first_frame(int W, int H, const float* depth_cur, float* depth_state, float* mask_out, cudaStream_t st);
 cudaError_t ggt_launch_weight_maps(const GgtWeightParams& p, cudaStream_t st);
-cudaError_t ggt_launch_integrate(const GgtIntegrateParams& p, int dtype, bool fused, cudaStream_t st);
+cudaError_t ggt_launch_integrate(const GgtIntegrateParams& p, int dtype, bool fused, int sm_count, cudaStream_t st);
 cudaError_t ggt_launch_temporal_weight(const GgtTemporalParams& p, cudaStream_t st);
 cudaError_t ggt_launch_features(const GgtFeatureParams& p, cudaStream_t st);
 cudaError_t ggt_launch_raymarch(const GgtRaymarchParams& p, cudaStream_t st);
