@@ -47,6 +47,8 @@ extern "C" {
 #define GGT_OVERWRITE 0u   /* T = sum(w c)/sum(w), W = sum(w)  (Eq. 10, normalised: reading P2) */
 #define GGT_ACCUMULATE 1u  /* running average against the stored {T, W} with decay and cap (P9) */
 
+#define GGT_FRAME_RESULTS_ASYNC 0x100u /* ggt_frame_host only, OR-ed into flags: result copies on the context's own stream */
+
 #define GGT_MAX_VIEWS 16
 #define GGT_MAX_BINS 1024
 
@@ -112,19 +114,22 @@ int ggt_selftest_arith(ggt_ctx* ctx, int64_t n, const float* dev_a, const float*
 /* Bytes of device scratch ggt_integrate needs for n_views maps of width x height: 8 B per record of the
  * zero-padded (height+1) x (width+1) {depth, omega} map, each map rounded up to 256 B. */
 size_t ggt_workspace_bytes(int32_t n_views, int32_t width, int32_t height);
-/* Hands caller-owned device scratch to the context.  Without it (or if it is too small) ggt_integrate
- * grows an internal cudaMalloc'ed buffer, which synchronises the device once per growth. */
+/* Hands caller-owned device scratch (256-B aligned) to the context.  Without it ggt_integrate grows an internal
+ * cudaMalloc'ed buffer, which synchronises the device once per growth; WITH it, a call whose views need more than
+ * `bytes` fails with GGT_ERR_SHAPE (the library never replaces a caller's buffer).  NULL hands the job back to the
+ * library. */
 int ggt_set_workspace(ggt_ctx* ctx, void* dev_workspace, size_t bytes);
 
 /* ---- volume ------------------------------------------------------------------------------------- */
 /* Bytes the caller must allocate for a volume: a 256-B-aligned table header (z_j, tau_j) followed by
  * the voxels in the internal layout  T[ceil(D/G)][H_t][W_t][G]  then  W[ceil(D/G)][H_t][W_t][G]  with G = 4 (fp32)
  * or 8 (fp16) bins per 128-bit access (bins are padded to a multiple of G), followed by one
- * 16-bit search hint per target ray (written by ggt_integrate*, read by ggt_extract_depth: the first group of bins
- * that holds a non-positive T).  The storage is opaque: only the ggt_* calls may write it. */
+ * 32-bit search range per target ray (written by ggt_integrate*, read by ggt_extract_depth: the first and last group
+ * of bins that hold an observed non-positive T).  The storage is opaque: only the ggt_* calls may write it. */
 size_t ggt_volume_bytes(const ggt_volume_desc* desc);
-/* Binds caller-owned device storage (>= ggt_volume_bytes, 256-B aligned) and uploads the bin tables
- * (synchronous small copy).  The storage content is otherwise untouched: call ggt_volume_reset. */
+/* Binds caller-owned device storage (>= ggt_volume_bytes, 256-B aligned) and uploads the bin tables (a small copy,
+ * complete on return whatever stream later calls use).  The storage content is otherwise untouched: call
+ * ggt_volume_reset. */
 int ggt_volume_bind(ggt_ctx* ctx, const ggt_volume_desc* desc, void* dev_storage, size_t bytes,
                     ggt_volume** out);
 int ggt_volume_unbind(ggt_ctx* ctx, ggt_volume* vol);
@@ -341,7 +346,16 @@ int ggt_guidance_features(ggt_ctx* ctx, const ggt_camera* target, const float* d
  *                     (bit 0: slot has history, bit 1: ping-pong parity).  A slot without history gets the
  *                     first-frame rule (M = 1).
  *   dev_staging       caller-owned device memory, >= ggt_frame_staging_bytes, 256-B aligned.
- *   host_depth / host_conf  fp32 H_t x W_t results (host; either may be NULL). */
+ *   host_depth / host_conf  fp32 H_t x W_t results (host; either may be NULL).
+ *   flags             GGT_OVERWRITE or GGT_ACCUMULATE, optionally | GGT_FRAME_RESULTS_ASYNC: the device -> host result
+ *                     copies then run on a stream of the context, out of two alternating sets of device buffers, so that the
+ *                     next call's kernels do not wait behind them on `stream`; the results of all such calls made so far
+ *                     are on the host once a stream that ggt_frame_host_results_wait(ctx, that stream) was called on has
+ *                     been synchronised.  The host result buffers of two consecutive calls must differ.
+ * Slots: the slots of one call must be distinct (GGT_ERR_INVALID_ARG otherwise).  host_slot_state is updated only when
+ * the whole call has been enqueued successfully.  A slot's history is whatever frame it last took part in: callers that
+ * want Eq. 2 against frame t-1 for every rig camera (as the paper refines all N views every frame) pass
+ * every rig view each frame; a camera that re-enters after a gap is blended against its older state. */
 size_t ggt_frame_staging_bytes(const ggt_volume_desc* desc, int32_t n_slots, int32_t n_views, int32_t width,
                                int32_t height);
 int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
@@ -349,6 +363,8 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
                    const int32_t* slots, int32_t n_slots, uint32_t* host_slot_state,
                    const ggt_refine_params* params, uint32_t flags, void* dev_staging, size_t staging_bytes,
                    float* host_depth, float* host_conf, void* stream);
+/* Makes `stream` wait (on the device) for the result copies of every GGT_FRAME_RESULTS_ASYNC call made so far. */
+int ggt_frame_host_results_wait(ggt_ctx* ctx, void* stream);
 
 #ifdef __cplusplus
 }

@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libggt.so")
 GGT_OK = 0
 GGT_F32, GGT_F16 = 0, 1
 GGT_OVERWRITE, GGT_ACCUMULATE = 0, 1
+GGT_FRAME_RESULTS_ASYNC = 0x100
 GGT_MAX_VIEWS = 16
 GGT_PROFILE_STAGES = 5
 
@@ -26,7 +27,7 @@ EXPORTS = [
     "ggt_volume_bytes", "ggt_volume_bind", "ggt_volume_unbind", "ggt_volume_reset", "ggt_volume_export",
     "ggt_volume_tables", "ggt_refine_depth", "ggt_refine_depth_batch", "ggt_integrate", "ggt_integrate_batch", "ggt_integrate_extract_batch", "ggt_extract_depth", "ggt_integrate_extract",
     "ggt_raymarch_depth", "ggt_guidance_features", "ggt_temporal_weight", "ggt_integrate_weighted", "ggt_raymarch_depth_weighted",
-    "ggt_frame_staging_bytes", "ggt_frame_host",
+    "ggt_frame_staging_bytes", "ggt_frame_host", "ggt_frame_host_results_wait",
     "ggt_splat_forward", "ggt_splat_reserve", "ggt_splat_status", "ggt_temporal_weight_mask",
 ]
 
@@ -126,6 +127,7 @@ def load_library() -> ctypes.CDLL:
                                              vp, vp]
     lib.ggt_frame_staging_bytes.argtypes = [descp, i32, i32, i32, i32]
     lib.ggt_frame_staging_bytes.restype = ctypes.c_size_t
+    lib.ggt_frame_host_results_wait.argtypes = [vp, vp]
     lib.ggt_frame_host.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), ctypes.POINTER(vp),
                                    ctypes.POINTER(i32), i32, ctypes.POINTER(u32),
                                    ctypes.POINTER(ggt_refine_params), u32, vp, ctypes.c_size_t, vp, vp, vp]
@@ -145,6 +147,30 @@ def to_camera(c) -> ggt_camera:
 
 def _ptr(t) -> Optional[int]:
     return None if t is None else t.data_ptr()
+
+
+def _chk(t, dtype, numel=None, what="tensor", cuda=True):
+    """Marshalling guard: the C ABI takes raw pointers, so dtype / device / layout / size are checked here."""
+    if t is None:
+        return None
+    import torch
+    want = getattr(torch, dtype)
+    if t.dtype != want:
+        raise GgtError("%s: dtype %s, expected %s" % (what, t.dtype, want))
+    if cuda and not t.is_cuda:
+        raise GgtError("%s: must be a CUDA tensor" % what)
+    if not cuda and (t.is_cuda or not t.is_pinned()):
+        raise GgtError("%s: must be a pinned host tensor" % what)
+    if not t.is_contiguous():
+        raise GgtError("%s: must be contiguous" % what)
+    if numel is not None and t.numel() != int(numel):
+        raise GgtError("%s: %d elements, expected %d" % (what, t.numel(), int(numel)))
+    return t
+
+
+def _chk_views(views, tensors, dtype="float32", what="depth"):
+    for k, (c, t) in enumerate(zip(views, tensors)):
+        _chk(t, dtype, int(c.width) * int(c.height), "%s of view %d" % (what, k))
 
 
 def _stream() -> int:
@@ -221,8 +247,11 @@ class Context:
         """In-place update of `depth_state` (torch fp32 HxW, cuda).  rgb_*: torch uint8 HxWx{3,4} or None."""
         H, W = depth_cur.shape
         stride = 3 if rgb_cur is None else int(rgb_cur.shape[2])
-        for t in (rgb_cur, rgb_prev, depth_cur, depth_state, mask_out, pooled_out):
-            assert t is None or (t.is_cuda and t.is_contiguous())
+        for t, nm in ((rgb_cur, "rgb_cur"), (rgb_prev, "rgb_prev")):
+            _chk(t, "uint8", H * W * stride, nm)
+        for t, nm in ((depth_cur, "depth_cur"), (depth_state, "depth_state"), (mask_out, "mask_out")):
+            _chk(t, "float32", H * W, nm)
+        _chk(pooled_out, "uint16", ((H + 3) // 4) * ((W + 3) // 4), "pooled_out")
         prm = _refine_params(lambda_t, beta, theta, downscale, pool)
         rc = self.lib.ggt_refine_depth(self.h, W, H, _ptr(rgb_cur), _ptr(rgb_prev), stride, _ptr(depth_cur),
                                        _ptr(depth_state), _ptr(mask_out), _ptr(pooled_out), ctypes.byref(prm),
@@ -241,6 +270,11 @@ class Context:
             if lst is None:
                 return None
             return (ctypes.c_void_p * V)(*[None if t is None else t.data_ptr() for t in lst])
+        for lst, dt, n in ((rgb_cur, "uint8", H * W * stride), (rgb_prev, "uint8", H * W * stride), (depth_cur, "float32", H * W),
+                           (depth_state, "float32", H * W), (mask_out, "float32", H * W),
+                           (pooled_out, "uint16", ((H + 3) // 4) * ((W + 3) // 4))):
+            for t in (lst or []):
+                _chk(t, dt, n, "ggt_refine_depth_batch argument")
         prm = _refine_params(lambda_t, beta, theta, downscale, pool)
         rc = self.lib.ggt_refine_depth_batch(self.h, V, W, H, arr(rgb_cur), arr(rgb_prev), stride, arr(depth_cur),
                                              arr(depth_state), arr(mask_out), arr(pooled_out), ctypes.byref(prm), _stream())
@@ -261,8 +295,7 @@ class Context:
     def ggt_integrate(self, vol: "Volume", target, views: Sequence, depths: Sequence, flags=GGT_OVERWRITE):
         V = len(views)
         t, arr = self._cams(target, views)
-        for d in depths:
-            assert d.is_cuda and d.is_contiguous() and d.dtype.is_floating_point
+        _chk_views(views, depths)
         ptrs = (ctypes.c_void_p * V)(*[d.data_ptr() for d in depths])
         rc = self.lib.ggt_integrate(self.h, vol.h, ctypes.byref(t), V, arr, ptrs, flags, _stream())
         self.check(rc, "ggt_integrate")
@@ -275,6 +308,7 @@ class Context:
         tarr = (ggt_camera * T)(*[to_camera(c) for c in targets])
         rarr = (ggt_camera * R)(*[to_camera(c) for c in rig_views])
         varr = (ctypes.c_void_p * T)(*[v.h for v in vols])
+        _chk_views(rig_views, depths)
         ptrs = (ctypes.c_void_p * R)(*[d.data_ptr() for d in depths])
         idx = (ctypes.c_int32 * (T * V))(*[int(i) for row in view_index for i in row])
         rc = self.lib.ggt_integrate_batch(self.h, T, varr, tarr, R, rarr, ptrs, V, idx, flags, _stream())
@@ -288,6 +322,10 @@ class Context:
         tarr = (ggt_camera * T)(*[to_camera(c) for c in targets])
         rarr = (ggt_camera * R)(*[to_camera(c) for c in rig_views])
         varr = (ctypes.c_void_p * T)(*[v.h for v in vols])
+        _chk_views(rig_views, depths)
+        for lst, dt in ((depth, "float32"), (conf, "float32"), (bins, "int32")):
+            for t, c in zip(lst or [], targets):
+                _chk(t, dt, int(c.width) * int(c.height), "ggt_integrate_extract_batch output")
         ptrs = (ctypes.c_void_p * R)(*[d.data_ptr() for d in depths])
         idx = (ctypes.c_int32 * (T * V))(*[int(i) for row in view_index for i in row])
 
@@ -301,13 +339,23 @@ class Context:
                               conf=None, bins=None):
         V = len(views)
         t, arr = self._cams(target, views)
+        _chk_views(views, depths)
+        self._chk_outputs(target, depth, conf, bins)
         ptrs = (ctypes.c_void_p * V)(*[d.data_ptr() for d in depths])
         rc = self.lib.ggt_integrate_extract(self.h, vol.h, ctypes.byref(t), V, arr, ptrs, flags, _ptr(depth),
                                             _ptr(conf), _ptr(bins), _stream())
         self.check(rc, "ggt_integrate_extract")
 
     # ---- a7 ----------------------------------------------------------------------------------------
+    @staticmethod
+    def _chk_outputs(target, depth, conf, ints):
+        n = int(target.width) * int(target.height)
+        _chk(depth, "float32", n, "depth output")
+        _chk(conf, "float32", n, "confidence output")
+        _chk(ints, "int32", n, "bin / steps output")
+
     def ggt_extract_depth(self, vol: "Volume", depth=None, conf=None, bins=None):
+        self._chk_outputs(vol, depth, conf, bins)
         rc = self.lib.ggt_extract_depth(self.h, vol.h, _ptr(depth), _ptr(conf), _ptr(bins), _stream())
         self.check(rc, "ggt_extract_depth")
 
@@ -317,6 +365,8 @@ class Context:
                            w_window=7):
         V = len(views)
         t, arr = self._cams(target, views)
+        _chk_views(views, depths)
+        self._chk_outputs(target, depth, conf, steps)
         ptrs = (ctypes.c_void_p * V)(*[d.data_ptr() for d in depths])
         prm = ggt_raymarch_params(z_near, z_far, tau, step_scale, min_step, max_evals, n_bisect, w_sigma0, w_clip, w_window)
         rc = self.lib.ggt_raymarch_depth(self.h, ctypes.byref(t), V, arr, ptrs, ctypes.byref(prm), _ptr(depth), _ptr(conf),
@@ -327,6 +377,10 @@ class Context:
     def ggt_temporal_weight(self, prev_target, prev_depth, prev_conf, views, masks, weight_out, beta=1.0, eta=15.0):
         V = len(views)
         t, arr = self._cams(prev_target, views if V else [prev_target])
+        n = int(prev_target.width) * int(prev_target.height)
+        for x, nm in ((prev_depth, "prev_depth"), (prev_conf, "prev_conf"), (weight_out, "weight_out")):
+            _chk(x, "float32", n, nm)
+        _chk_views(views, masks, what="mask")
         ptrs = (ctypes.c_void_p * max(V, 1))(*[m.data_ptr() for m in masks])
         rc = self.lib.ggt_temporal_weight(self.h, ctypes.byref(t), prev_depth.data_ptr(), prev_conf.data_ptr(), V, arr, ptrs,
                                           beta, eta, weight_out.data_ptr(), _stream())
@@ -341,6 +395,8 @@ class Context:
     def ggt_integrate_weighted(self, vol: "Volume", target, views, depths, weights, flags=GGT_OVERWRITE):
         V = len(views)
         t, arr = self._cams(target, views)
+        _chk_views(views, depths)
+        _chk_views(views, weights or [], what="weights")
         ptrs = (ctypes.c_void_p * V)(*[d.data_ptr() for d in depths])
         rc = self.lib.ggt_integrate_weighted(self.h, vol.h, ctypes.byref(t), V, arr, ptrs, self._weight_ptrs(weights, V), flags,
                                              _stream())
@@ -351,6 +407,9 @@ class Context:
                                     w_clip=0.02, w_window=7):
         V = len(views)
         t, arr = self._cams(target, views)
+        _chk_views(views, depths)
+        _chk_views(views, weights or [], what="weights")
+        self._chk_outputs(target, depth, conf, steps)
         ptrs = (ctypes.c_void_p * V)(*[d.data_ptr() for d in depths])
         prm = ggt_raymarch_params(z_near, z_far, tau, step_scale, min_step, max_evals, n_bisect, w_sigma0, w_clip, w_window)
         rc = self.lib.ggt_raymarch_depth_weighted(self.h, ctypes.byref(t), V, arr, ptrs, self._weight_ptrs(weights, V),
@@ -362,6 +421,10 @@ class Context:
                           out_mask=None, out_count=None, sigma_px=0.5, dilation=0.3, z_cull=0.2):
         t, arr = self._cams(target, [view])
         stride = 3 if rgb is None else int(rgb.shape[2])
+        ns, nt = int(view.width) * int(view.height), int(target.width) * int(target.height)
+        _chk(depth, "float32", ns, "depth"); _chk(rgb, "uint8", ns * stride, "rgb"); _chk(mask, "float32", ns, "mask")
+        _chk(out_rgb, "float32", 3 * nt, "out_rgb"); _chk(out_alpha, "float32", nt, "out_alpha")
+        _chk(out_depth, "float32", nt, "out_depth"); _chk(out_mask, "float32", nt, "out_mask"); _chk(out_count, "int32", nt, "out_count")
         prm = ggt_splat_params(sigma_px, dilation, z_cull, 0)
         rc = self.lib.ggt_splat_forward(self.h, ctypes.byref(t), arr, depth.data_ptr(), _ptr(rgb), stride, _ptr(mask),
                                         ctypes.byref(prm), _ptr(out_rgb), _ptr(out_alpha), _ptr(out_depth), _ptr(out_mask),
@@ -379,6 +442,8 @@ class Context:
 
     def ggt_temporal_weight_mask(self, prev_depth, prev_conf, masks, weight_out, beta=1.0, eta=15.0):
         K = len(masks)
+        for x in [prev_depth, prev_conf, weight_out] + list(masks):
+            _chk(x, "float32", prev_depth.numel(), "ggt_temporal_weight_mask argument")
         ptrs = (ctypes.c_void_p * K)(*[m.data_ptr() for m in masks])
         rc = self.lib.ggt_temporal_weight_mask(self.h, prev_depth.numel(), prev_depth.data_ptr(), prev_conf.data_ptr(), K, ptrs,
                                                beta, eta, weight_out.data_ptr(), _stream())
@@ -388,6 +453,9 @@ class Context:
     def ggt_guidance_features(self, target, depth, views, features):
         V = len(views)
         t, arr = self._cams(target, views)
+        n = int(target.width) * int(target.height)
+        _chk(depth, "float32", n, "depth")
+        _chk(features, "float32", 4 * V * n, "features")
         rc = self.lib.ggt_guidance_features(self.h, ctypes.byref(t), depth.data_ptr(), V, arr, features.data_ptr(), _stream())
         self.check(rc, "ggt_guidance_features")
 
@@ -398,6 +466,14 @@ class Context:
         """host_* are pinned CPU torch tensors; slot_state is a numpy uint32 array kept by the caller."""
         V = len(views)
         t, arr = self._cams(target, views)
+        for k, c in enumerate(views):
+            n = int(c.width) * int(c.height)
+            _chk(host_depth_in[k], "float32", n, "host depth of view %d" % k, cuda=False)
+            if host_rgb is not None:
+                _chk(host_rgb[k], "uint8", 3 * n, "host colour of view %d" % k, cuda=False)
+        nt = int(target.width) * int(target.height)
+        _chk(host_depth, "float32", nt, "host_depth", cuda=False); _chk(host_conf, "float32", nt, "host_conf", cuda=False)
+        _chk(staging, "uint8", None, "staging")
         rgbp = None
         if host_rgb is not None:
             rgbp = (ctypes.c_void_p * V)(*[None if r is None else r.data_ptr() for r in host_rgb])
@@ -409,6 +485,10 @@ class Context:
             ctypes.byref(refine_params) if refine_params is not None else None, flags, staging.data_ptr(),
             staging.numel(), _ptr(host_depth), _ptr(host_conf), _stream())
         self.check(rc, "ggt_frame_host")
+
+    def ggt_frame_host_results_wait(self):
+        """The current stream waits for the result copies of all GGT_FRAME_RESULTS_ASYNC calls made so far."""
+        self.check(self.lib.ggt_frame_host_results_wait(self.h, _stream()), "ggt_frame_host_results_wait")
 
 
 class Volume:

@@ -97,7 +97,7 @@ size_t voxel_bytes_of(const ggt_volume_desc* d) {
     return align_up((size_t)ng * d->width * d->height * 32, 256);     // one 128-bit word per group and pixel in each of the two planes
 }
 
-size_t hint_bytes_of(const ggt_volume_desc* d) { return align_up((size_t)d->width * d->height * sizeof(uint16_t), 256); }
+size_t hint_bytes_of(const ggt_volume_desc* d) { return align_up((size_t)d->width * d->height * sizeof(uint32_t), 256); }
 
 }  // namespace
 
@@ -138,6 +138,9 @@ int ggt_destroy(ggt_ctx* ctx) {
     if (c->ev_inputs_free) cudaEventDestroy(c->ev_inputs_free);
     if (c->ev_h2d_done) cudaEventDestroy(c->ev_h2d_done);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->ev_kernels_done) cudaEventDestroy(c->ev_kernels_done);
+    for (int i = 0; i < 2; ++i) if (c->ev_d2h_done[i]) cudaEventDestroy(c->ev_d2h_done[i]);
+    if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
     delete c;
     return GGT_OK;
 }
@@ -232,7 +235,7 @@ int ggt_volume_bind(ggt_ctx* ctx, const ggt_volume_desc* desc, void* dev_storage
     v->dev_tables = static_cast<float*>(dev_storage);
     v->dev_voxels = static_cast<char*>(dev_storage) + v->header_bytes;
     v->hint_bytes = hint_bytes_of(desc);
-    v->dev_hints = reinterpret_cast<uint16_t*>(static_cast<char*>(dev_storage) + v->header_bytes + v->voxel_bytes);
+    v->dev_hints = reinterpret_cast<uint32_t*>(static_cast<char*>(dev_storage) + v->header_bytes + v->voxel_bytes);
     const int Dpad = v->n_groups * v->group;
     std::vector<float> tab(2 * (size_t)Dpad);
     for (int j = 0; j < Dpad; ++j) {
@@ -241,7 +244,10 @@ int ggt_volume_bind(ggt_ctx* ctx, const ggt_volume_desc* desc, void* dev_storage
         tab[j] = v->z[j < D ? j : D - 1];
         tab[Dpad + j] = j < D ? v->tau[j] : -1e30f;
     }
+    // pageable source: cudaMemcpy may return while the DMA is still in flight, and the kernels that read the tables run on
+    // the caller's (possibly non-blocking) streams, so wait for the legacy stream the copy ran on
     cudaError_t e = cudaMemcpy(v->dev_tables, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(nullptr);
     if (e != cudaSuccess) { delete v; return cuda_fail(ctx, e, "upload of bin tables"); }
     *out = v;
     return GGT_OK;
@@ -254,7 +260,7 @@ int ggt_volume_unbind(ggt_ctx*, ggt_volume* vol) {
 
 int ggt_volume_reset(ggt_ctx* ctx, ggt_volume* vol, void* stream) {
     if (!ctx || !vol) return GGT_ERR_INVALID_ARG;
-    // voxels and, right behind them, the per-ray search hints (0 = search everything)
+    // voxels and, right behind them, the per-ray search ranges (0 = empty: an all-zero volume has no crossing)
     cudaError_t e = cudaMemsetAsync(vol->dev_voxels, 0, vol->voxel_bytes + vol->hint_bytes, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "volume reset");
     ctx->launches += 1;
@@ -778,14 +784,24 @@ int ggt_guidance_features(ggt_ctx* ctx, const ggt_camera* target, const float* d
 // staging layout (every block 256-B aligned), all views width x height:
 //   per slot s:  rgb[2][H*W*3] (ping-pong current / previous colour), state[H*W] fp32 refined depth
 //   per view k:  depth_cur[H*W] fp32
-//   outputs:     depth[Ht*Wt], conf[Ht*Wt] fp32
+//   outputs:     two sets of depth[Ht*Wt], conf[Ht*Wt] fp32 (alternating, see GGT_FRAME_RESULTS_ASYNC)
 size_t ggt_frame_staging_bytes(const ggt_volume_desc* desc, int32_t n_slots, int32_t n_views, int32_t width,
                                int32_t height) {
     if (!desc || n_slots <= 0 || n_views <= 0 || width <= 0 || height <= 0) return 0;
     const size_t px = (size_t)width * height;
     const size_t rgb = align_up(px * 3, 256), dep = align_up(px * 4, 256);
     const size_t out = align_up((size_t)desc->width * desc->height * 4, 256);
-    return (size_t)n_slots * (2 * rgb + dep) + (size_t)n_views * dep + 2 * out;
+    return (size_t)n_slots * (2 * rgb + dep) + (size_t)n_views * dep + 4 * out;
+}
+
+int ggt_frame_host_results_wait(ggt_ctx* ctx, void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    for (int i = 0; i < 2; ++i) {
+        if (!ctx->d2h_pending[i]) continue;
+        cudaError_t e = cudaStreamWaitEvent((cudaStream_t)stream, ctx->ev_d2h_done[i], 0);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "ggt_frame_host_results_wait");
+    }
+    return GGT_OK;
 }
 
 int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
@@ -802,7 +818,12 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
         if (views[k].width != W || views[k].height != H) return fail(ctx, GGT_ERR_SHAPE, "ggt_frame_host needs equal view sizes");
         if (slots[k] < 0 || slots[k] >= n_slots) return fail(ctx, GGT_ERR_INVALID_ARG, "slots[%d] = %d", k, slots[k]);
         if (!host_depth_cur[k]) return fail(ctx, GGT_ERR_INVALID_ARG, "host_depth_cur[%d] is NULL", k);
+        for (int j = 0; j < k; ++j)
+            if (slots[j] == slots[k]) return fail(ctx, GGT_ERR_INVALID_ARG, "slots[%d] == slots[%d] = %d: two views of one call cannot share a history slot", j, k, slots[k]);
     }
+    const bool async_results = (flags & GGT_FRAME_RESULTS_ASYNC) != 0;
+    flags &= ~GGT_FRAME_RESULTS_ASYNC;
+    if (flags != GGT_OVERWRITE && flags != GGT_ACCUMULATE) return fail(ctx, GGT_ERR_INVALID_ARG, "flags %u", flags);
     if (((uintptr_t)dev_staging & 255) != 0) return fail(ctx, GGT_ERR_INVALID_ARG, "staging must be 256-byte aligned");
     const size_t need = ggt_frame_staging_bytes(&vol->desc, n_slots, n_views, W, H);
     if (staging_bytes < need) return fail(ctx, GGT_ERR_SHAPE, "staging %zu B < required %zu B", staging_bytes, need);
@@ -831,6 +852,7 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
     const float* dptr[GGT_MAX_VIEWS];
     uint8_t* rcur[GGT_MAX_VIEWS];
     const uint8_t* rprev[GGT_MAX_VIEWS];
+    uint32_t new_state[GGT_MAX_VIEWS];                 // committed to host_slot_state only once every enqueue has succeeded
     for (int k = 0; k < n_views; ++k) {
         char* slot = base + (size_t)slots[k] * (2 * rgb + dep);
         float* dcur = reinterpret_cast<float*>(view_base + (size_t)k * dep);
@@ -838,13 +860,13 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
         if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D depth");
         rcur[k] = nullptr; rprev[k] = nullptr;
         if (refine && host_rgb_cur[k]) {
-            uint32_t& s = host_slot_state[slots[k]];          // bit 0: has history, bit 1: parity of "current"
+            const uint32_t s = host_slot_state[slots[k]];     // bit 0: has history, bit 1: parity of "current"
             const int cur = (s >> 1) & 1 ? 0 : 1;
             rcur[k] = reinterpret_cast<uint8_t*>(slot + (size_t)cur * rgb);
             rprev[k] = (s & 1) ? reinterpret_cast<const uint8_t*>(slot + (size_t)(1 - cur) * rgb) : nullptr;
             e = cudaMemcpyAsync(rcur[k], host_rgb_cur[k], px * 3, cudaMemcpyHostToDevice, cs);
             if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D colour");
-            s = 1u | ((uint32_t)cur << 1);
+            new_state[k] = 1u | ((uint32_t)cur << 1);
         }
     }
     {
@@ -852,6 +874,7 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
         if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ctx->ev_h2d_done, 0);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D event");
     }
+    bool all_refined = false;
     {   // all refined views in one batched call (two launches for the frame)
         const uint8_t* bc[GGT_MAX_VIEWS]; const uint8_t* bp[GGT_MAX_VIEWS];
         const float* bd[GGT_MAX_VIEWS]; float* bs[GGT_MAX_VIEWS];
@@ -871,10 +894,28 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
             int rcode = ggt_refine_depth_batch(ctx, nb, W, H, bc, bp, 3, bd, bs, nullptr, nullptr, params, stream);
             if (rcode != GGT_OK) return rcode;
         }
+        all_refined = nb == n_views;
     }
-    float* d_depth = reinterpret_cast<float*>(out_base);
-    float* d_conf = reinterpret_cast<float*>(out_base + out);
-    ctx->record_inputs_free = true;
+    if (all_refined) {     // every uploaded buffer has been consumed by the refine kernels (the weight maps read the states)
+        cudaError_t e = cudaEventRecord(ctx->ev_inputs_free, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "event record");
+        ctx->inputs_free_pending = true;
+    }
+    // results: set 0, or alternating sets when their copies run on the context's own stream
+    if (async_results && !ctx->d2h_stream) {
+        cudaError_t e = cudaStreamCreateWithFlags(&ctx->d2h_stream, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_kernels_done, cudaEventDisableTiming);
+        for (int i = 0; i < 2 && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&ctx->ev_d2h_done[i], cudaEventDisableTiming);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "result stream / events");
+    }
+    const int set = async_results ? ctx->result_set : 0;
+    if (ctx->d2h_pending[set]) {                         // the kernels below overwrite this set: its last copy must be done
+        cudaError_t e = cudaStreamWaitEvent(st, ctx->ev_d2h_done[set], 0);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "stream wait");
+    }
+    float* d_depth = reinterpret_cast<float*>(out_base + (size_t)set * 2 * out);
+    float* d_conf = reinterpret_cast<float*>(out_base + (size_t)set * 2 * out + out);
+    ctx->record_inputs_free = !all_refined;       // else: the weight-map pre-pass is the last reader of the uploads
     // a3-a7 in one pass: the result the host wants comes out of the integrate kernel itself (same bits as
     // ggt_integrate followed by ggt_extract_depth, without re-reading the volume)
     int rcode = ggt_integrate_extract(ctx, vol, target, n_views, views, dptr, flags, host_depth ? d_depth : nullptr,
@@ -882,14 +923,29 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
     ctx->record_inputs_free = false;
     if (rcode != GGT_OK) return rcode;
     const size_t ob = (size_t)vol->desc.width * vol->desc.height * 4;
+    cudaStream_t rs = st;
+    if (async_results) {
+        rs = ctx->d2h_stream;
+        cudaError_t e = cudaEventRecord(ctx->ev_kernels_done, st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(rs, ctx->ev_kernels_done, 0);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "result event");
+    }
     if (host_depth) {
-        cudaError_t e = cudaMemcpyAsync(host_depth, d_depth, ob, cudaMemcpyDeviceToHost, st);
+        cudaError_t e = cudaMemcpyAsync(host_depth, d_depth, ob, cudaMemcpyDeviceToHost, rs);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "D2H depth");
     }
     if (host_conf) {
-        cudaError_t e = cudaMemcpyAsync(host_conf, d_conf, ob, cudaMemcpyDeviceToHost, st);
+        cudaError_t e = cudaMemcpyAsync(host_conf, d_conf, ob, cudaMemcpyDeviceToHost, rs);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "D2H confidence");
     }
+    if (async_results) {
+        cudaError_t e = cudaEventRecord(ctx->ev_d2h_done[set], rs);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "result event");
+        ctx->d2h_pending[set] = true;
+        ctx->result_set ^= 1;
+    }
+    for (int k = 0; k < n_views; ++k)                  // every enqueue succeeded: the slots now hold this frame
+        if (rcur[k]) host_slot_state[slots[k]] = new_state[k];
     return GGT_OK;
 }
 

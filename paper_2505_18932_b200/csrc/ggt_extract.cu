@@ -4,9 +4,10 @@
 //
 // One thread per target ray.  The volume is two planes per group, [group][v][u] x {G values of T} and the same for
 // W (G = 4 bins fp32, 8 bins fp16): the search reads the T plane only (128-bit words, 512 contiguous bytes per warp
-// request), UNROLL groups ahead, starting at the per-ray hint k_integrate left (the first group with a bin T <= 0),
+// request), UNROLL groups ahead, over the per-ray range k_integrate left (the groups with an observed bin T <= 0),
 // and fetches weights just for the candidates; after each batch a warp vote (__all_sync) ends the march for the warp
-// once all 32 rays have their crossing: a warp reads the groups between its front-most hint and its last crossing.
+// once all 32 rays have their crossing: a warp reads the groups between its front-most hint and its last crossing
+// (or the rear-most hint of the rays that have none).
 #include "ggt_internal.h"
 
 
@@ -59,12 +60,15 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
     // The search runs on the T plane alone (half of the volume's bytes): a candidate is T_{j-1} > 0 >= T_j; only then
     // are the two weights fetched, and the candidate is a crossing if both bins were observed (reading P13).  An
     // unobserved bin holds T = 0, so it ends a positive run as a candidate and is then rejected by its W = 0.
-    // k_integrate left, per ray, the first group that holds a bin with T <= 0 (n_groups: none; 0 after a reset).  The
-    // far bin of a crossing is such a bin, so the search starts one group before the hint: the front-most hint of the
-    // warp's 32 rays, to keep its loads coalesced.  A ray without such a bin has no crossing.
-    const int my_hint = live ? (int)__ldg(p.hint + ((size_t)v * p.Wt + u)) : p.n_groups;
-    const int g_start = max((int)__reduce_min_sync(0xffffffffu, (unsigned)my_hint) - 1, 0) / UNROLL * UNROLL;
-    bool found = !live || my_hint >= p.n_groups;
+    // k_integrate left, per ray, the range of groups that hold an observed bin with T <= 0 (first | end << 16; end <=
+    // first: none).  The far bin of a crossing is such a bin, so the search runs from one group before the first to the
+    // last one -- for the warp, from the front-most start to the rear-most end of its 32 rays, which keeps the loads
+    // coalesced.  A ray with an empty range has no crossing.
+    const uint32_t hw = live ? __ldg(p.hint + ((size_t)v * p.Wt + u)) : 0u;
+    const int h_first = (int)(hw & 0xffffu), h_end = min((int)(hw >> 16), p.n_groups);
+    bool found = !live || h_end <= h_first;
+    const int g_start = max((int)__reduce_min_sync(0xffffffffu, found ? 0xffffu : (unsigned)h_first) - 1, 0) / UNROLL * UNROLL;
+    const int g_end = (int)__reduce_max_sync(0xffffffffu, found ? 0u : (unsigned)h_end);
     float pT = 0.0f;
     float out_d = 0.0f, out_c = 0.0f;
     int out_b = -1;
@@ -90,11 +94,11 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
         }
     };
     uint32_t ppos = 0, plast = 0;                        // fp16: "> 0" mask and raw bits of the previous half2
-    for (int g = g_start; g < p.n_groups; g += UNROLL) {
+    for (int g = g_start; g < g_end; g += UNROLL) {
         uint4 w[UNROLL];
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q)
-            w[q] = (g + q < p.n_groups && !found) ? __ldcs(tpl + (size_t)(g + q) * plane) : make_uint4(0, 0, 0, 0);
+            w[q] = (g + q < g_end && !found) ? __ldcs(tpl + (size_t)(g + q) * plane) : make_uint4(0, 0, 0, 0);
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q) {
             if (HALF) {
@@ -122,6 +126,7 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
                 pT = d;
             }
         }
+        found = found || g + UNROLL >= h_end;            // every group of this ray's range has been searched
         if (__all_sync(0xffffffffu, found)) break;
     }
     if (!live) return;

@@ -31,7 +31,7 @@ struct GgtIntegrateParams {
     unsigned long long plane;   // Wt * Ht: 128-bit words per group of the volume
     const float* tables;   // device: z[0..Dpad) then tau[0..Dpad), Dpad = n_groups * G
     void* voxels;          // device: T[n_groups][Ht][Wt][G] then W[n_groups][Ht][Wt][G]
-    uint16_t* hint;        // device: per ray, first group holding a bin with T <= 0 (n_groups = none): ggt_extract_depth's start
+    uint32_t* hint;        // device: per ray, first | (last + 1) << 16 of the groups holding an observed bin with T <= 0
     float* depth;          // fused extract outputs (may be null)
     float* conf;
     int32_t* bin;
@@ -143,7 +143,7 @@ struct GgtExtractParams {
     int32_t Wt, Ht, D, n_groups;
     const float* tables;
     const void* voxels;
-    const uint16_t* hint;  // per ray search hint written by k_integrate (0 after a reset: search everything)
+    const uint32_t* hint;  // per ray search range written by k_integrate (0 after a reset: nothing to find)
     float* depth;
     float* conf;
     int32_t* bin;
@@ -173,6 +173,12 @@ struct ggt_ctx {
     cudaEvent_t ev_inputs_free = nullptr, ev_h2d_done = nullptr;
     bool inputs_free_pending = false;
     bool record_inputs_free = false;
+    // GGT_FRAME_RESULTS_ASYNC: the device -> host result copies run on d2h_stream out of two alternating sets of device
+    // result buffers, so the next frame's kernels do not queue behind them on the caller's stream
+    cudaStream_t d2h_stream = nullptr;
+    cudaEvent_t ev_kernels_done = nullptr, ev_d2h_done[2] = {nullptr, nullptr};
+    bool d2h_pending[2] = {false, false};
+    int result_set = 0;
     // optional per-stage device timing (ggt_profile_enable): pairs of events around each kernel group
     bool prof = false;
     struct ProfRec { int stage; cudaEvent_t a, b; };
@@ -191,7 +197,7 @@ struct ggt_volume {
     size_t voxel_bytes = 0;
     float* dev_tables = nullptr;   // inside the caller's storage
     void* dev_voxels = nullptr;    // inside the caller's storage
-    uint16_t* dev_hints = nullptr; // inside the caller's storage, after the voxels: one search hint per ray
+    uint32_t* dev_hints = nullptr; // inside the caller's storage, after the voxels: one search range per ray
     size_t hint_bytes = 0;
 };
 

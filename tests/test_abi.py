@@ -42,12 +42,12 @@ def test_volume_bytes_layout():
         d = binding.ggt_volume_desc(1920, 1080, 128, z.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), 2.0, 0.0,
                                     0.001, 0.02, 7, 64.0, 1.0, dtype)
         n = lib.ggt_volume_bytes(ctypes.byref(d))
-        # table header (2 x 128 floats) + the two planes + one 16-bit search hint per ray, each block 256-B aligned
-        assert n == 1024 + 1920 * 1080 * 128 * per_voxel + 1920 * 1080 * 2
+        # table header (2 x 128 floats) + the two planes + one 32-bit search range per ray, each block 256-B aligned
+        assert n == 1024 + 1920 * 1080 * 128 * per_voxel + 1920 * 1080 * 4
     # ragged bin count pads to the 128-bit group
     d = binding.ggt_volume_desc(10, 10, 33, z.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), 2.0, 0.0, 0.001, 0.02,
                                 7, 64.0, 1.0, binding.GGT_F16)
-    assert lib.ggt_volume_bytes(ctypes.byref(d)) == 512 + 16128 + 256      # 33 bins -> 5 groups of 8: 16000 B of voxels (rounded up to 256), 200 B of hints
+    assert lib.ggt_volume_bytes(ctypes.byref(d)) == 512 + 16128 + 512      # 33 bins -> 5 groups of 8: 16000 B of voxels (rounded up to 256), 400 B of hints
     assert lib.ggt_workspace_bytes(4, 1920, 1080) == 4 * (-(-(1921 * 1081 * 8) // 256) * 256)
 
 

@@ -309,9 +309,31 @@ def test_frame_host_pipelined_without_host_sync():
     for f in range(F):                                   # no synchronise inside the loop
         ctx.ggt_frame_host(vol, tgt, views, rgb[f], dep[f], vi, state, staging, outs[f][0], outs[f][1], refine_params=prm)
     torch.cuda.synchronize()
+    refs = [gp.frame(f)[0] for f in range(F)]
+    refs = [(r["depth"].cpu(), r["conf"].cpu()) for r in refs]
     for f in range(F):
-        ref = gp.frame(f)[0]
-        assert torch.equal(outs[f][0], ref["depth"].cpu()) and torch.equal(outs[f][1], ref["conf"].cpu()), "frame %d" % f
+        assert torch.equal(outs[f][0], refs[f][0]) and torch.equal(outs[f][1], refs[f][1]), "frame %d" % f
+    # the same stream of frames with the result copies on the context's own stream (GGT_FRAME_RESULTS_ASYNC): the caller's
+    # stream is synchronised only after ggt_frame_host_results_wait; two host result buffers alternate
+    ctx2 = binding.Context()
+    vol2 = ctx2.ggt_volume_bind(tgt.width, tgt.height, wl.z_bins)
+    state2 = np.zeros(n_slots, np.uint32)
+    two = [(torch.empty(n, dtype=torch.float32).pin_memory(), torch.empty(n, dtype=torch.float32).pin_memory()) for _ in range(2)]
+    got = []
+    for f in range(F):
+        ctx2.ggt_frame_host(vol2, tgt, views, rgb[f], dep[f], vi, state2, staging, two[f & 1][0], two[f & 1][1],
+                            flags=binding.GGT_OVERWRITE | binding.GGT_FRAME_RESULTS_ASYNC, refine_params=prm)
+        if f % 2 == 1:                                   # read both buffers back every second frame
+            ctx2.ggt_frame_host_results_wait()
+            torch.cuda.current_stream().synchronize()
+            got += [(two[0][0].clone(), two[0][1].clone()), (two[1][0].clone(), two[1][1].clone())]
+    for f in range(F):
+        assert torch.equal(got[f][0], refs[f][0]) and torch.equal(got[f][1], refs[f][1]), "async frame %d" % f
+    # duplicate history slots in one call are rejected, and a failed call leaves the slot state untouched
+    before = state2.copy()
+    with pytest.raises(binding.GgtError):
+        ctx2.ggt_frame_host(vol2, tgt, views, rgb[0], dep[0], [vi[0]] * len(vi), state2, staging, two[0][0], two[0][1], refine_params=prm)
+    assert np.array_equal(before, state2)
 
 
 def test_refine_batch_equals_per_view_and_oracle():

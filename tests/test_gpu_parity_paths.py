@@ -277,3 +277,25 @@ def test_refine_accepts_unaligned_depth_pointers():
     torch.cuda.synchronize()
     assert np.array_equal(sg.cpu().numpy().view(np.uint32), o_out.view(np.uint32))
     assert np.array_equal(Mg.cpu().numpy().view(np.uint32), o_M.view(np.uint32))
+
+
+def test_binding_rejects_wrong_dtype_device_layout_and_size():
+    """the C ABI takes raw pointers: the binding refuses tensors that would be silently reinterpreted"""
+    import torch
+    from paper_2505_18932_b200 import binding
+    wl, tgt, views = _grid_case()
+    z = synth.bins_inverse(0.5, 5, 16)
+    ctx = binding.Context()
+    vol = ctx.ggt_volume_bind(tgt.width, tgt.height, z)
+    good = [torch.ones((c.height, c.width), device="cuda") for c in views]
+    ctx.ggt_integrate(vol, tgt, views, good)
+    for bad in (good[0].double(), good[0].half(), good[0].cpu(), good[0][:, :-1], good[0].t()):
+        with pytest.raises(binding.GgtError):
+            ctx.ggt_integrate(vol, tgt, views, [bad] + good[1:])
+    n = tgt.width * tgt.height
+    with pytest.raises(binding.GgtError):
+        ctx.ggt_extract_depth(vol, torch.empty(n - 1, device="cuda"))
+    with pytest.raises(binding.GgtError):
+        ctx.ggt_extract_depth(vol, torch.empty(n, device="cuda"), bins=torch.empty(n, dtype=torch.int64, device="cuda"))
+    with pytest.raises(binding.GgtError):
+        ctx.ggt_raymarch_depth(tgt, views, [g.double() for g in good], 0.5, 5.0, depth=torch.empty(n, device="cuda"))
