@@ -32,6 +32,20 @@ def test_T23_exp_le0_against_numpy():
     assert np.all(np.diff(vals) >= 0)
 
 
+def test_T23_alpha_threshold_is_a_single_crossing_in_q():
+    """alpha >= 1/255 (reading S4) as a threshold on q: with the fp32 exponential of S8 the decision is exactly
+    q >= q* = -5.541263580322266 (0xC0B15208).  Checked on EVERY float of [-5.56, -5.52]; outside, exp(q) is more than
+    2 % away from 1/255 and the exponential is good to 1e-6.  (The CUDA scatter passes use this form.)"""
+    qstar = np.float32(-5.541263580322266)
+    assert qstar.view(np.uint32) == 0xC0B15208
+    thr = np.float32(1.0) / np.float32(255.0)
+    bits = np.arange(int(np.float32(-5.52).view(np.uint32)), int(np.float32(-5.56).view(np.uint32)) + 1, dtype=np.uint32)
+    qs = bits.view(np.float32)
+    ge = np.array([np.float32(oracle.exp_le0(float(q))) >= thr for q in qs])
+    assert np.array_equal(ge, qs >= qstar) and ge.any() and not ge.all()
+    assert math.exp(-5.52) > 1.02 / 255 and math.exp(-5.56) < 0.99 / 255
+
+
 # ---- T24: one Gaussian in closed form ------------------------------------------------------------------------------------
 def test_T24_single_gaussian_footprint_and_peak():
     c = cam()
