@@ -427,10 +427,12 @@ static void detect_fast_paths(GgtIntegrateParams& p, int32_t n_views) {
     p.same_size = 1;
     for (int k = 1; k < n_views; ++k)
         if (p.v[k].width != p.v[0].width || p.v[k].height != p.v[0].height) p.same_size = 0;
-    // parallel rig: w_k(z) = fma(z, fma(h20, uc, fma(h21, vc, h22)), e2) has the same bits in every view
+    // rig of identical parallel cameras with coplanar centres: H_k and e_k[2] have the same bits in every view, so
+    // b_k = H_k (uc, vc, 1) and w_k(z) = fma(z, b_k[2], e2) do too
     p.shared_w = p.same_size && n_views >= 2;
     for (int k = 1; k < n_views; ++k)
-        if (memcmp(p.v[k].h2, p.v[0].h2, sizeof p.v[0].h2) != 0 || memcmp(&p.v[k].e2, &p.v[0].e2, sizeof(float)) != 0) p.shared_w = 0;
+        if (memcmp(p.v[k].nh, p.v[0].nh, sizeof p.v[0].nh) != 0 || memcmp(p.v[k].h2, p.v[0].h2, sizeof p.v[0].h2) != 0 ||
+            memcmp(&p.v[k].e2, &p.v[0].e2, sizeof(float)) != 0) p.shared_w = 0;
 }
 
 // Shared front end of ggt_integrate / ggt_integrate_extract: validation, workspace, weight maps, launch.

@@ -26,7 +26,7 @@ struct GgtIntegrateParams {
     int32_t n_groups;      // ceil(D / G)
     int32_t accumulate;    // 0 overwrite, 1 running average
     int32_t same_size;     // 1 if all views have the same width x height
-    int32_t shared_w;      // 1 if additionally row 2 of H_k and e_k[2] are bit-identical in all views (n_views >= 2)
+    int32_t shared_w;      // 1 if additionally H_k and e_k[2] are bit-identical in all views (n_views >= 2)
     float decay, cap;
     unsigned long long plane;   // Wt * Ht: 128-bit words per group of the volume
     const float* tables;   // device: z[0..Dpad) then tau[0..Dpad), Dpad = n_groups * G
