@@ -264,3 +264,39 @@ def test_temporal_weight_from_a_splatted_mask_closed_form():
     w = oracle.temporal_weight_mask(d, conf, M, beta=0.5, eta=15.0)
     # min(beta omega_acc max(1 - M, 0), eta): 0.5*4*0.4 | M = 1 -> 0 | no depth | no weight | capped at eta | M > 1 -> 0
     assert np.allclose(w, [0.8, 0.0, 0.0, 0.0, 15.0, 0.0], atol=1e-6)
+
+
+# ---- F1's gather and the paper's splat-and-max differ exactly where a surface point is occluded in an input view ------------
+def test_splatted_mask_differs_from_the_gather_at_occluded_points():
+    """Eq. 13's novel-view mask two ways (readings F1 and S1-S8).  A moving foreground strip (mask 1) in front
+    of a static wall (mask 0.6), one input view 20 cm to the side of the camera of D^{t-1}.  For wall points that the
+    strip hides from the input view, the gather (orc_temporal_weight) projects the wall point into the view and reads
+    the STRIP's mask, so the static wall loses its temporal weight; the splat composites the view's own surfaces front
+    to back, nothing of the view lands on those pixels, and the weight survives.  Everywhere else the two agree."""
+    W, H, f = 96, 24, 100.0
+    prev = cam(W=W, H=H, f=f)
+    view = cam(centre=(0.2, 0, 0), W=W, H=H, f=f)
+    scene = synth.Scene(3.0, [synth.Primitive("box", np.array([0.0, 0.0, 1.0]), np.array([0.08, 2.0, 0.001]), np.zeros(3), np.zeros(9))])
+    d_prev = synth.raycast(prev, scene)[0].astype(np.float32)
+    d_view = synth.raycast(view, scene)[0].astype(np.float32)
+    m_view = np.where(d_view < 2.0, 1.0, 0.6).astype(np.float32)          # the strip moved, the wall did not
+    conf = np.full((H, W), 4.0, np.float32)
+    w_gather = oracle.temporal_weight(prev, d_prev, conf, [view], [m_view], beta=1.0, eta=15.0)
+    sp = oracle.splat_forward(prev, view, d_view, mask=m_view)
+    w_splat = oracle.temporal_weight_mask(d_prev, conf, sp["mask"], beta=1.0, eta=15.0)
+    row = H // 2
+    wall = d_prev[row] > 2.0
+    # wall pixels of D^{t-1} whose surface point projects onto the strip in the input view: hidden from it
+    x_in_view = (np.arange(W) + 0.5 - prev.cx) / f * 3.0 - 0.2              # world x of the wall point, relative to the view
+    u_view = np.floor(x_in_view / 3.0 * f + view.cx).astype(int)
+    hidden = wall & (u_view >= 0) & (u_view < W)
+    hidden[hidden] = d_view[row, u_view[hidden]] < 2.0
+    assert hidden.sum() >= 4
+    assert np.allclose(w_gather[row, hidden], 0.0)                          # the gather read the occluder's mask (M = 1)
+    inner = hidden & np.roll(hidden, 2) & np.roll(hidden, -2)               # away from the splats' 2-px tails
+    assert inner.sum() >= 1 and np.allclose(w_splat[row, inner], 4.0)       # nothing of the view lands there: M = 0
+    # a wall point both cameras see, far from the strip: both give beta * omega_acc * (1 - 0.6)
+    far = wall & ~hidden & (np.abs(np.arange(W) - W // 2) > 30) & (u_view >= 3) & (u_view < W - 3)
+    assert far.sum() > 10
+    assert np.allclose(w_gather[row, far], 1.6, atol=1e-5) and np.allclose(w_splat[row, far], 4.0 * (1 - 0.6 * sp["alpha"][row, far]), atol=1e-4)
+    assert np.abs(w_splat[row, far] - 1.6).max() < 0.01
