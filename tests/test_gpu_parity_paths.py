@@ -299,3 +299,49 @@ def test_binding_rejects_wrong_dtype_device_layout_and_size():
         ctx.ggt_extract_depth(vol, torch.empty(n, device="cuda"), bins=torch.empty(n, dtype=torch.int64, device="cuda"))
     with pytest.raises(binding.GgtError):
         ctx.ggt_raymarch_depth(tgt, views, [g.double() for g in good], 0.5, 5.0, depth=torch.empty(n, device="cuda"))
+
+
+# ---- the per-ray search ranges that ggt_integrate* leaves for ggt_extract_depth --------------------------------------------
+def test_extract_after_reset_fused_and_large_unsplit_launches():
+    """ggt_extract_depth relies on the search range every volume writer leaves per ray: a reset volume has nothing to find,
+    a volume written by the fused call is searched in full, and an unsplit launch (image large enough for gridDim.z = 1)
+    writes real ranges -- each must give exactly what the oracle's full search gives."""
+    import torch
+    from paper_2505_18932_b200 import binding
+    wl = synth.workload("C2", scale=0.5)                      # 320 x 180: the launch is not split over the bin range
+    tgt = wl.targets(0)[0]
+    vi = wl.views_for(tgt)
+    views = [wl.rig[v] for v in vi]
+    depths = [wl.view_inputs(0, v)[0] for v in vi]
+    tau = oracle.tau_table(wl.z_bins, wl.trunc_bins)
+    T, W = oracle.integrate(tgt, wl.z_bins, tau, views, [oracle.weight_map(d) for d in depths])
+    od, oc, ob = oracle.extract(wl.z_bins, T, W)
+    ctx = binding.Context()
+    n = tgt.width * tgt.height
+    gd = [torch.from_numpy(np.array(d)).cuda() for d in depths]
+    out = lambda: (torch.empty(n, device="cuda"), torch.empty(n, device="cuda"), torch.empty(n, dtype=torch.int32, device="cuda"))
+    for dtype in (binding.GGT_F32, binding.GGT_F16):
+        vol = ctx.ggt_volume_bind(tgt.width, tgt.height, wl.z_bins, dtype=dtype)
+        vol.ggt_volume_reset()
+        d0, c0, b0 = out()
+        ctx.ggt_extract_depth(vol, d0, c0, b0)
+        assert bool((b0 == -1).all()) and bool((d0 == 0).all())
+        if dtype == binding.GGT_F16:
+            T16, W16 = oracle.integrate(tgt, wl.z_bins, tau, views, [oracle.weight_map(d) for d in depths], half_storage=True)
+            ed, ec, eb = oracle.extract(wl.z_bins, T16, W16)
+        else:
+            ed, ec, eb = od, oc, ob
+        # fused writer, then a separate search of the same volume
+        d1, c1, b1 = out()
+        ctx.ggt_integrate_extract(vol, tgt, views, gd, binding.GGT_OVERWRITE, d1, c1, b1)
+        d2, c2, b2 = out()
+        ctx.ggt_extract_depth(vol, d2, c2, b2)
+        # plain writer (real ranges), then the search
+        ctx.ggt_integrate(vol, tgt, views, gd)
+        d3, c3, b3 = out()
+        ctx.ggt_extract_depth(vol, d3, c3, b3)
+        for d, c, b in ((d1, c1, b1), (d2, c2, b2), (d3, c3, b3)):
+            assert np.array_equal(b.cpu().numpy(), eb)
+            assert np.array_equal(d.cpu().numpy().view(np.uint32), ed.view(np.uint32))
+            assert np.array_equal(c.cpu().numpy().view(np.uint32), ec.view(np.uint32))
+    assert (ob >= 0).mean() > 0.5 and (ob < 0).any()
