@@ -37,6 +37,8 @@
 // closed-form evaluation counts), T15-T18 temporal weight (Eq. 13 closed forms, fp64 brute-force mask gather,
 // Eq. 14 recursion in closed form, variance reduction), T19-T22 network-input features (plane / sphere normals,
 // fp64 ray dot products and constant maps, undefined pixels).
+// The forward warp with pixel-sized Gaussians (row f-3) and Eq. 13 from a splatted mask live in ggt_oracle_splat.cpp (the
+// second source file of this library; pins T23-T28 in tests/test_oracle_splat_pins.py).
 // Parity unpinned (choices, not derivable): the VALUES of tau in C2-C5 (P3), the
 // dead-zone threshold semantics (P6), decay/cap without mask gate (P9-P10), the border rule of
 // Eq. 12 (P11), the confidence output (P13); in orc_raymarch the min_step / max_evals / unobserved-sample
