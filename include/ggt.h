@@ -333,9 +333,10 @@ int ggt_guidance_features(ggt_ctx* ctx, const ggt_camera* target, const float* d
 
 /* ---- end-to-end frame from HOST buffers (bench.py "e2e") ----------------------------------------- */
 /* One whole frame through the three steps with host<->device copies inside the call, enqueued without
- * synchronising: kernels and the result copies on `stream`; the input uploads on a copy stream owned by the
- * context, which `stream` waits for (events), so consecutive calls overlap frame n + 1's uploads with frame n's
- * kernels.  The host input buffers must stay valid until `stream` has passed this call's kernels; the results
+ * synchronising: kernels on `stream`; the input uploads and the result copies on two streams owned by the context,
+ * ordered against `stream` with events.  Within a frame each view's refine kernels and weight map start as soon as
+ * that view's upload has landed, and the fused integrate / extract kernel runs as four row slices whose results
+ * travel while the next slice computes; consecutive calls overlap frame n + 1's uploads with frame n's kernels.  The host input buffers must stay valid until `stream` has passed this call's kernels; the results
  * are complete when `stream` is synchronised.  All n_views views must have the same width x height.
  *   host_rgb_cur[k]   uint8 HxWx3 colour of view k at this frame (host; array or entry may be NULL -> that
  *                     view is not refined, its depth is used as is); params NULL also disables refinement.

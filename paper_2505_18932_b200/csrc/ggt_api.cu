@@ -137,6 +137,7 @@ int ggt_destroy(ggt_ctx* ctx) {
     for (auto& r : c->prof_pool) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     if (c->ev_inputs_free) cudaEventDestroy(c->ev_inputs_free);
     if (c->ev_h2d_done) cudaEventDestroy(c->ev_h2d_done);
+    for (int i = 0; i < GGT_MAX_VIEWS; ++i) if (c->ev_view[i]) cudaEventDestroy(c->ev_view[i]);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->ev_kernels_done) cudaEventDestroy(c->ev_kernels_done);
     for (int i = 0; i < 2; ++i) if (c->ev_d2h_done[i]) cudaEventDestroy(c->ev_d2h_done[i]);
@@ -358,7 +359,7 @@ int ggt_refine_depth(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t*
 // (one launch); map_out[k] is the device address of view k's zero-padded {depth, omega} map.
 static int prepare_maps(ggt_ctx* ctx, int32_t n_views, const ggt_camera* views, const float* const* dev_depths,
                         const float* const* dev_weights, float w_sigma0, float w_clip, int32_t w_window,
-                        const float2** map_out, cudaStream_t st) {
+                        const float2** map_out, cudaStream_t st, int only_view = -1) {
     size_t need = 0;
     for (int k = 0; k < n_views; ++k) {
         if (views[k].width <= 0 || views[k].height <= 0 || views[k].width > 32767 || views[k].height > 32767)
@@ -387,6 +388,11 @@ static int prepare_maps(ggt_ctx* ctx, int32_t n_views, const ggt_camera* views, 
         wp.v[k].weight = dev_weights ? dev_weights[k] : nullptr;
         wp.v[k].width = views[k].width; wp.v[k].height = views[k].height;
         w += align_up(((size_t)views[k].width + 1) * ((size_t)views[k].height + 1) * sizeof(float2), 256);
+    }
+    if (ctx->weights_prelaunched) return GGT_OK;      // ggt_frame_host launched them view by view, behind each view's upload
+    if (only_view >= 0) {                               // one view of the set (same workspace layout)
+        wp.v[0] = wp.v[only_view];
+        wp.n_views = 1;
     }
     cudaError_t e = ggt_launch_weight_maps(wp, st);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "weight-map launch");
@@ -436,10 +442,13 @@ static void detect_fast_paths(GgtIntegrateParams& p, int32_t n_views) {
 }
 
 // Shared front end of ggt_integrate / ggt_integrate_extract: validation, workspace, weight maps, launch.
+// ggt_frame_host launches a frame in row slices so that each slice's results can travel while the next one computes
+struct SliceHook { int (*fn)(void* user, int row0, int row1); void* user; int n_slices; };
+
 static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int32_t n_views,
                           const ggt_camera* views, const float* const* dev_depths, const float* const* dev_weights,
                           uint32_t flags, bool fused,
-                          float* dev_depth, float* dev_conf, int32_t* dev_bin, void* stream) {
+                          float* dev_depth, float* dev_conf, int32_t* dev_bin, void* stream, const SliceHook* hook = nullptr) {
     if (!ctx) return GGT_ERR_INVALID_ARG;
     if (!vol || !target || !views || !dev_depths) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL volume / camera / depth pointer");
     if (n_views < 1 || n_views > GGT_MAX_VIEWS) return fail(ctx, GGT_ERR_SHAPE, "n_views %d not in [1, %d]", n_views, GGT_MAX_VIEWS);
@@ -465,9 +474,19 @@ static int integrate_impl(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* targe
     }
     StageTimer tm(ctx, GGT_STAGE_INTEGRATE, st);
     detect_fast_paths(p, n_views);
-    cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, fused, ctx->sm_count, st);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "integrate launch");
-    ctx->launches += 1;
+    const int n_slices = hook ? hook->n_slices : 1;
+    for (int sl = 0; sl < n_slices; ++sl) {
+        p.row0 = (int)((long long)p.Ht * sl / n_slices) / 8 * 8;              // whole CTAs of 8 rows
+        p.row1 = sl + 1 == n_slices ? p.Ht : (int)((long long)p.Ht * (sl + 1) / n_slices) / 8 * 8;
+        if (p.row1 <= p.row0) continue;
+        cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, fused, ctx->sm_count, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "integrate launch");
+        ctx->launches += 1;
+        if (hook) {
+            const int rc = hook->fn(hook->user, p.row0, p.row1);
+            if (rc != GGT_OK) return rc;
+        }
+    }
     return GGT_OK;
 }
 
@@ -537,6 +556,7 @@ static int integrate_batch_impl(ggt_ctx* ctx, int32_t n_targets, ggt_volume* con
             fill_view_params(targets[t], rig_views[idx], maps[idx], p.v[k]);
         }
         detect_fast_paths(p, n_views);
+        p.row0 = 0; p.row1 = p.Ht;
         StageTimer tm(ctx, GGT_STAGE_INTEGRATE, st);
         cudaError_t e = ggt_launch_integrate(p, vol->desc.dtype, fused, ctx->sm_count, st);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "integrate launch");
@@ -855,12 +875,15 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
     uint8_t* rcur[GGT_MAX_VIEWS];
     const uint8_t* rprev[GGT_MAX_VIEWS];
     uint32_t new_state[GGT_MAX_VIEWS];                 // committed to host_slot_state only once every enqueue has succeeded
+    // view by view: its uploads on the copy stream, and -- as soon as they have landed -- its refine kernels and its
+    // weight map on the caller's stream, so that only the last view's small kernels are left after the last upload
     for (int k = 0; k < n_views; ++k) {
         char* slot = base + (size_t)slots[k] * (2 * rgb + dep);
         float* dcur = reinterpret_cast<float*>(view_base + (size_t)k * dep);
         cudaError_t e = cudaMemcpyAsync(dcur, host_depth_cur[k], px * 4, cudaMemcpyHostToDevice, cs);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D depth");
         rcur[k] = nullptr; rprev[k] = nullptr;
+        dptr[k] = dcur;
         if (refine && host_rgb_cur[k]) {
             const uint32_t s = host_slot_state[slots[k]];     // bit 0: has history, bit 1: parity of "current"
             const int cur = (s >> 1) & 1 ? 0 : 1;
@@ -869,42 +892,45 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
             e = cudaMemcpyAsync(rcur[k], host_rgb_cur[k], px * 3, cudaMemcpyHostToDevice, cs);
             if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D colour");
             new_state[k] = 1u | ((uint32_t)cur << 1);
+            dptr[k] = reinterpret_cast<float*>(slot + 2 * rgb);          // the slot's refined-depth state
         }
-    }
-    {
-        cudaError_t e = cudaEventRecord(ctx->ev_h2d_done, cs);
-        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ctx->ev_h2d_done, 0);
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "H2D event");
-    }
-    bool all_refined = false;
-    {   // all refined views in one batched call (two launches for the frame)
-        const uint8_t* bc[GGT_MAX_VIEWS]; const uint8_t* bp[GGT_MAX_VIEWS];
-        const float* bd[GGT_MAX_VIEWS]; float* bs[GGT_MAX_VIEWS];
-        int nb = 0;
-        for (int k = 0; k < n_views; ++k) {
-            char* slot = base + (size_t)slots[k] * (2 * rgb + dep);
-            float* state = reinterpret_cast<float*>(slot + 2 * rgb);
-            float* dcur = reinterpret_cast<float*>(view_base + (size_t)k * dep);
-            if (rcur[k]) {
-                bc[nb] = rcur[k]; bp[nb] = rprev[k]; bd[nb] = dcur; bs[nb] = state; ++nb;
-                dptr[k] = state;
-            } else {
-                dptr[k] = dcur;
-            }
+        if (!ctx->ev_view[k]) {
+            e = cudaEventCreateWithFlags(&ctx->ev_view[k], cudaEventDisableTiming);
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "view event");
         }
-        if (nb > 0) {
-            int rcode = ggt_refine_depth_batch(ctx, nb, W, H, bc, bp, 3, bd, bs, nullptr, nullptr, params, stream);
+        e = cudaEventRecord(ctx->ev_view[k], cs);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "view event");
+    }
+    for (int k = 0; k < n_views; ++k) {
+        cudaError_t e = cudaStreamWaitEvent(st, ctx->ev_view[k], 0);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "view event wait");
+        if (rcur[k]) {
+            const uint8_t* bc = rcur[k]; const uint8_t* bp = rprev[k];
+            const float* bd = reinterpret_cast<const float*>(view_base + (size_t)k * dep);
+            float* bs = const_cast<float*>(dptr[k]);
+            int rcode = ggt_refine_depth_batch(ctx, 1, W, H, &bc, &bp, 3, &bd, &bs, nullptr, nullptr, params, stream);
             if (rcode != GGT_OK) return rcode;
         }
-        all_refined = nb == n_views;
+        // the last reader of the uploaded buffers is the last view's refine kernel (its weight map reads the slot's state)
+        // or, for a view that is not refined, its weight map: from there on the next frame's uploads may overwrite them
+        const bool last = k == n_views - 1;
+        if (last && rcur[k]) {
+            e = cudaEventRecord(ctx->ev_inputs_free, st);
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "event record");
+        }
+        const float2* maps_unused[GGT_MAX_VIEWS];
+        int rcode = prepare_maps(ctx, n_views, views, dptr, nullptr, vol->desc.w_sigma0, vol->desc.w_clip, vol->desc.w_window,
+                                 maps_unused, st, k);
+        if (rcode != GGT_OK) return rcode;
+        if (last && !rcur[k]) {
+            e = cudaEventRecord(ctx->ev_inputs_free, st);
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "event record");
+        }
     }
-    if (all_refined) {     // every uploaded buffer has been consumed by the refine kernels (the weight maps read the states)
-        cudaError_t e = cudaEventRecord(ctx->ev_inputs_free, st);
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "event record");
-        ctx->inputs_free_pending = true;
-    }
-    // results: set 0, or alternating sets when their copies run on the context's own stream
-    if (async_results && !ctx->d2h_stream) {
+    ctx->inputs_free_pending = true;
+    // results: their copies run on the context's own stream, slice by slice behind the kernels that produce them; set 0,
+    // or alternating sets of device buffers when the caller does not wait for them (GGT_FRAME_RESULTS_ASYNC)
+    if (!ctx->d2h_stream) {
         cudaError_t e = cudaStreamCreateWithFlags(&ctx->d2h_stream, cudaStreamNonBlocking);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_kernels_done, cudaEventDisableTiming);
         for (int i = 0; i < 2 && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&ctx->ev_d2h_done[i], cudaEventDisableTiming);
@@ -917,34 +943,39 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
     }
     float* d_depth = reinterpret_cast<float*>(out_base + (size_t)set * 2 * out);
     float* d_conf = reinterpret_cast<float*>(out_base + (size_t)set * 2 * out + out);
-    ctx->record_inputs_free = !all_refined;       // else: the weight-map pre-pass is the last reader of the uploads
+    ctx->weights_prelaunched = true;
     // a3-a7 in one pass: the result the host wants comes out of the integrate kernel itself (same bits as
-    // ggt_integrate followed by ggt_extract_depth, without re-reading the volume)
-    int rcode = ggt_integrate_extract(ctx, vol, target, n_views, views, dptr, flags, host_depth ? d_depth : nullptr,
-                                      host_conf ? d_conf : nullptr, nullptr, stream);
-    ctx->record_inputs_free = false;
+    // ggt_integrate followed by ggt_extract_depth, without re-reading the volume).  When the caller waits for the results
+    // on `stream`, the frame runs as 4 row slices: slice i's results cross PCIe while slice i + 1 computes.
+    struct CopyCtx { ggt_ctx* ctx; cudaStream_t st; float *dd, *dc, *hd, *hc; int Wt; } cc = {ctx, st, d_depth, d_conf, host_depth, host_conf, vol->desc.width};
+    SliceHook hook;
+    hook.user = &cc;
+    hook.n_slices = (async_results || (!host_depth && !host_conf)) ? 1 : 4;
+    hook.fn = [](void* user, int row0, int row1) -> int {
+        CopyCtx& c = *static_cast<CopyCtx*>(user);
+        cudaStream_t rs = c.ctx->d2h_stream;
+        cudaError_t e = cudaEventRecord(c.ctx->ev_kernels_done, c.st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(rs, c.ctx->ev_kernels_done, 0);
+        const size_t o = (size_t)row0 * c.Wt, nb = (size_t)(row1 - row0) * c.Wt * sizeof(float);
+        if (e == cudaSuccess && c.hd) e = cudaMemcpyAsync(c.hd + o, c.dd + o, nb, cudaMemcpyDeviceToHost, rs);
+        if (e == cudaSuccess && c.hc) e = cudaMemcpyAsync(c.hc + o, c.dc + o, nb, cudaMemcpyDeviceToHost, rs);
+        return e == cudaSuccess ? GGT_OK : cuda_fail(c.ctx, e, "D2H results");
+    };
+    int rcode = integrate_impl(ctx, vol, target, n_views, views, dptr, nullptr, flags, true, host_depth ? d_depth : nullptr,
+                               host_conf ? d_conf : nullptr, nullptr, stream, &hook);
+    ctx->weights_prelaunched = false;
     if (rcode != GGT_OK) return rcode;
-    const size_t ob = (size_t)vol->desc.width * vol->desc.height * 4;
-    cudaStream_t rs = st;
-    if (async_results) {
-        rs = ctx->d2h_stream;
-        cudaError_t e = cudaEventRecord(ctx->ev_kernels_done, st);
-        if (e == cudaSuccess) e = cudaStreamWaitEvent(rs, ctx->ev_kernels_done, 0);
+    {
+        cudaError_t e = cudaEventRecord(ctx->ev_d2h_done[set], ctx->d2h_stream);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "result event");
-    }
-    if (host_depth) {
-        cudaError_t e = cudaMemcpyAsync(host_depth, d_depth, ob, cudaMemcpyDeviceToHost, rs);
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "D2H depth");
-    }
-    if (host_conf) {
-        cudaError_t e = cudaMemcpyAsync(host_conf, d_conf, ob, cudaMemcpyDeviceToHost, rs);
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "D2H confidence");
-    }
-    if (async_results) {
-        cudaError_t e = cudaEventRecord(ctx->ev_d2h_done[set], rs);
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "result event");
-        ctx->d2h_pending[set] = true;
-        ctx->result_set ^= 1;
+        if (async_results) {
+            ctx->d2h_pending[set] = true;
+            ctx->result_set ^= 1;
+        } else {                                         // the results are complete when `stream` is synchronised
+            e = cudaStreamWaitEvent(st, ctx->ev_d2h_done[set], 0);
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "stream wait");
+            ctx->d2h_pending[set] = false;
+        }
     }
     for (int k = 0; k < n_views; ++k)                  // every enqueue succeeded: the slots now hold this frame
         if (rcur[k]) host_slot_state[slots[k]] = new_state[k];

@@ -27,6 +27,7 @@ struct GgtIntegrateParams {
     int32_t accumulate;    // 0 overwrite, 1 running average
     int32_t same_size;     // 1 if all views have the same width x height
     int32_t shared_w;      // 1 if additionally H_k and e_k[2] are bit-identical in all views (n_views >= 2)
+    int32_t row0, row1;    // target rows [row0, row1) this launch covers (ggt_frame_host slices a frame; else 0, Ht)
     float decay, cap;
     unsigned long long plane;   // Wt * Ht: 128-bit words per group of the volume
     const float* tables;   // device: z[0..Dpad) then tau[0..Dpad), Dpad = n_groups * G
@@ -173,6 +174,8 @@ struct ggt_ctx {
     cudaEvent_t ev_inputs_free = nullptr, ev_h2d_done = nullptr;
     bool inputs_free_pending = false;
     bool record_inputs_free = false;
+    cudaEvent_t ev_view[GGT_MAX_VIEWS] = {};   // ggt_frame_host: view k's uploads have landed
+    bool weights_prelaunched = false;          // ggt_frame_host launched the weight maps view by view already
     // GGT_FRAME_RESULTS_ASYNC: the device -> host result copies run on d2h_stream out of two alternating sets of device
     // result buffers, so the next frame's kernels do not queue behind them on the caller's stream
     cudaStream_t d2h_stream = nullptr;
