@@ -136,7 +136,6 @@ int ggt_destroy(ggt_ctx* ctx) {
     if (c->splat_flags) cudaFree(c->splat_flags);
     for (auto& r : c->prof_pool) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     if (c->ev_inputs_free) cudaEventDestroy(c->ev_inputs_free);
-    if (c->ev_h2d_done) cudaEventDestroy(c->ev_h2d_done);
     for (int i = 0; i < GGT_MAX_VIEWS; ++i) if (c->ev_view[i]) cudaEventDestroy(c->ev_view[i]);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->ev_kernels_done) cudaEventDestroy(c->ev_kernels_done);
@@ -397,11 +396,6 @@ static int prepare_maps(ggt_ctx* ctx, int32_t n_views, const ggt_camera* views, 
     cudaError_t e = ggt_launch_weight_maps(wp, st);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "weight-map launch");
     ctx->launches += 1;
-    if (ctx->record_inputs_free) {     // ggt_frame_host: the uploaded inputs are dead from here on
-        e = cudaEventRecord(ctx->ev_inputs_free, st);
-        if (e != cudaSuccess) return cuda_fail(ctx, e, "event record");
-        ctx->inputs_free_pending = true;
-    }
     return GGT_OK;
 }
 
@@ -863,7 +857,6 @@ int ggt_frame_host(ggt_ctx* ctx, ggt_volume* vol, const ggt_camera* target, int3
     if (!ctx->copy_stream) {
         cudaError_t e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_inputs_free, cudaEventDisableTiming);
-        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_h2d_done, cudaEventDisableTiming);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "copy stream / events");
     }
     cudaStream_t cs = ctx->copy_stream;

@@ -168,12 +168,11 @@ struct ggt_ctx {
     size_t splat_entries = 0;      // list capacity in entries (0 = automatic: 40 per source pixel)
     uint32_t* splat_flags = nullptr;
     // ggt_frame_host: host->device copies run on an internal stream so that the next frame's inputs upload while
-    // this frame's integrate / extract kernels run.  ev_inputs_free is recorded on the caller's stream once the
-    // weight-map pre-pass (the last kernel that reads the uploaded depth / colour buffers) has been enqueued.
+    // this frame's integrate / extract kernels run.  ev_inputs_free is recorded on the caller's stream behind the last
+    // kernel that reads the uploaded depth / colour buffers (the last view's refine kernel, or its weight map).
     cudaStream_t copy_stream = nullptr;
-    cudaEvent_t ev_inputs_free = nullptr, ev_h2d_done = nullptr;
+    cudaEvent_t ev_inputs_free = nullptr;
     bool inputs_free_pending = false;
-    bool record_inputs_free = false;
     cudaEvent_t ev_view[GGT_MAX_VIEWS] = {};   // ggt_frame_host: view k's uploads have landed
     bool weights_prelaunched = false;          // ggt_frame_host launched the weight maps view by view already
     // GGT_FRAME_RESULTS_ASYNC: the device -> host result copies run on d2h_stream out of two alternating sets of device

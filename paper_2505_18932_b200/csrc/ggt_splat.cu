@@ -345,12 +345,9 @@ cudaError_t ggt_launch_splat(const GgtSplatParams& p, cudaStream_t st, int* n_la
     k_scan_sums<<<1, SCAN_T, 0, st>>>(n_blocks, p.block_sums, p.total, p.capacity, p.overflow);
     k_scan_apply<<<n_blocks, SCAN_T, 0, st>>>(Nt, p.counts, p.block_sums, p.pos);
     k_splat_scatter<true><<<gs, blk, 0, st>>>(p);
-    static bool attr_set = false;                           // 64 KB of dynamic shared memory: opt in once
-    if (!attr_set) {
-        e = cudaFuncSetAttribute(k_splat_composite, cudaFuncAttributeMaxDynamicSharedMemorySize, kPool * (int)sizeof(uint2));
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    // 64 KB of dynamic shared memory needs the opt-in (per device and context, so it is simply set before every launch)
+    e = cudaFuncSetAttribute(k_splat_composite, cudaFuncAttributeMaxDynamicSharedMemorySize, kPool * (int)sizeof(uint2));
+    if (e != cudaSuccess) return e;
     k_splat_composite<<<gt, blk, kPool * sizeof(uint2), st>>>(p);
     *n_launches = 7;
     return cudaGetLastError();
