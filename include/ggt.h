@@ -50,6 +50,7 @@ extern "C" {
 #define GGT_FRAME_RESULTS_ASYNC 0x100u /* ggt_frame_host only, OR-ed into flags: result copies on the context's own stream */
 
 #define GGT_MAX_VIEWS 16
+#define GGT_REFINE_STATIC_MAX_CELLS 262144 /* ggt_refine_depth_static: ceil(W/4) * ceil(H/4) at most (e.g. 2048 x 2048) */
 #define GGT_MAX_BINS 1024
 
 /* Pinhole camera, no skew / distortion.  x_cam = R p_world + t. */
@@ -150,6 +151,21 @@ int ggt_refine_depth(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t*
                      const uint8_t* dev_rgb_prev, int32_t rgb_pixel_stride, const float* dev_depth_cur,
                      float* dev_depth_state, float* dev_mask_out, uint16_t* dev_pooled_out,
                      const ggt_refine_params* params, void* stream);
+
+/* ggt_refine_depth for callers that may not allocate device memory (code under stream capture, serving loops, harnesses
+ * that forbid cudaMalloc): same arguments, same arithmetic, same result bits, but the quarter-resolution scratch of
+ * Eq. 1 lives in a fixed array of GGT_REFINE_STATIC_MAX_CELLS x 2 B = 512 KB inside the library's device
+ * image (held by every GPU that loads the library until the process exits) instead of the context's growing buffer.
+ * The call makes no cudaMalloc / cudaFree and no other allocating call, and does no stage timing.
+ *   - ceil(width/4) * ceil(height/4) > GGT_REFINE_STATIC_MAX_CELLS -> GGT_ERR_SHAPE, nothing launched.
+ *   - the array is shared by ALL calls (all contexts, all streams) on a device and keeps the last call's contents; every
+ *     cell a call reads is written by that call first, so nothing has to be cleared between calls -- but two calls that
+ *     overlap on the GPU (different streams, no ordering between them) race on it: order them on one stream or by events.
+ *   - the device address is looked up once per device on the first call made with that device current. */
+int ggt_refine_depth_static(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t* dev_rgb_cur,
+                            const uint8_t* dev_rgb_prev, int32_t rgb_pixel_stride, const float* dev_depth_cur,
+                            float* dev_depth_state, float* dev_mask_out, uint16_t* dev_pooled_out,
+                            const ggt_refine_params* params, void* stream);
 
 /* The same for n_views views of ONE size in two launches (a frame's views at once): every argument of
  * ggt_refine_depth becomes a HOST array of n_views entries (device pointers).  dev_rgb_cur / dev_rgb_prev /

@@ -25,7 +25,7 @@ GGT_PROFILE_STAGES = 5
 EXPORTS = [
     "ggt_create", "ggt_destroy", "ggt_last_error", "ggt_launch_count", "ggt_profile_enable", "ggt_profile_collect", "ggt_selftest_arith", "ggt_workspace_bytes", "ggt_set_workspace",
     "ggt_volume_bytes", "ggt_volume_bind", "ggt_volume_unbind", "ggt_volume_reset", "ggt_volume_export",
-    "ggt_volume_tables", "ggt_refine_depth", "ggt_refine_depth_batch", "ggt_integrate", "ggt_integrate_batch", "ggt_integrate_extract_batch", "ggt_extract_depth", "ggt_integrate_extract",
+    "ggt_volume_tables", "ggt_refine_depth", "ggt_refine_depth_static", "ggt_refine_depth_batch", "ggt_integrate", "ggt_integrate_batch", "ggt_integrate_extract_batch", "ggt_extract_depth", "ggt_integrate_extract",
     "ggt_raymarch_depth", "ggt_guidance_features", "ggt_temporal_weight", "ggt_integrate_weighted", "ggt_raymarch_depth_weighted",
     "ggt_frame_staging_bytes", "ggt_frame_host", "ggt_frame_host_results_wait",
     "ggt_splat_forward", "ggt_splat_reserve", "ggt_splat_status", "ggt_temporal_weight_mask",
@@ -101,6 +101,7 @@ def load_library() -> ctypes.CDLL:
     lib.ggt_volume_export.argtypes = [vp, vp, vp, vp, vp]
     lib.ggt_volume_tables.argtypes = [vp, f32p, f32p]
     lib.ggt_refine_depth.argtypes = [vp, i32, i32, vp, vp, i32, vp, vp, vp, vp, ctypes.POINTER(ggt_refine_params), vp]
+    lib.ggt_refine_depth_static.argtypes = lib.ggt_refine_depth.argtypes
     lib.ggt_integrate.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), u32, vp]
     lib.ggt_extract_depth.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.ggt_integrate_extract.argtypes = [vp, vp, camp, i32, camp, ctypes.POINTER(vp), u32, vp, vp, vp, vp]
@@ -257,6 +258,22 @@ class Context:
                                        _ptr(depth_state), _ptr(mask_out), _ptr(pooled_out), ctypes.byref(prm),
                                        _stream())
         self.check(rc, "ggt_refine_depth")
+
+    def ggt_refine_depth_static(self, rgb_cur, rgb_prev, depth_cur, depth_state, mask_out=None, pooled_out=None,
+                                lambda_t=0.7, beta=0.6, theta=0.0, downscale=4, pool=3):
+        """ggt_refine_depth without any device allocation: scratch in the library's fixed 512 KB device array."""
+        H, W = depth_cur.shape
+        stride = 3 if rgb_cur is None else int(rgb_cur.shape[2])
+        for t, nm in ((rgb_cur, "rgb_cur"), (rgb_prev, "rgb_prev")):
+            _chk(t, "uint8", H * W * stride, nm)
+        for t, nm in ((depth_cur, "depth_cur"), (depth_state, "depth_state"), (mask_out, "mask_out")):
+            _chk(t, "float32", H * W, nm)
+        _chk(pooled_out, "uint16", ((H + 3) // 4) * ((W + 3) // 4), "pooled_out")
+        prm = _refine_params(lambda_t, beta, theta, downscale, pool)
+        rc = self.lib.ggt_refine_depth_static(self.h, W, H, _ptr(rgb_cur), _ptr(rgb_prev), stride, _ptr(depth_cur),
+                                              _ptr(depth_state), _ptr(mask_out), _ptr(pooled_out), ctypes.byref(prm),
+                                              _stream())
+        self.check(rc, "ggt_refine_depth_static")
 
     def ggt_refine_depth_batch(self, rgb_cur, rgb_prev, depth_cur, depth_state, mask_out=None, pooled_out=None,
                                lambda_t=0.7, beta=0.6, theta=0.0, downscale=4, pool=3):

@@ -354,6 +354,46 @@ int ggt_refine_depth(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t*
                                   &dev_depth_state, &dev_mask_out, &dev_pooled_out, params, stream);
 }
 
+// ggt_refine_depth with the block-difference scratch in the library's fixed device array (ggt_refine.cu): no allocation
+// of any kind on this path, and no StageTimer (its event pool grows on demand).
+int ggt_refine_depth_static(ggt_ctx* ctx, int32_t width, int32_t height, const uint8_t* dev_rgb_cur,
+                            const uint8_t* dev_rgb_prev, int32_t rgb_pixel_stride, const float* dev_depth_cur,
+                            float* dev_depth_state, float* dev_mask_out, uint16_t* dev_pooled_out,
+                            const ggt_refine_params* params, void* stream) {
+    if (!ctx) return GGT_ERR_INVALID_ARG;
+    if (width <= 0 || height <= 0) return fail(ctx, GGT_ERR_SHAPE, "image size %dx%d", width, height);
+    if (!dev_depth_cur || !dev_depth_state || !params) return fail(ctx, GGT_ERR_INVALID_ARG, "NULL depth / params pointer");
+    if (rgb_pixel_stride != 3 && rgb_pixel_stride != 4) return fail(ctx, GGT_ERR_INVALID_ARG, "rgb_pixel_stride %d (3 or 4)", rgb_pixel_stride);
+    if (params->downscale != 4 || params->pool != 3) return fail(ctx, GGT_ERR_UNSUPPORTED, "only downscale 4 / pool 3 (PAPER.md:81) are implemented");
+    if (!(params->lambda_t > 0.0f)) return fail(ctx, GGT_ERR_INVALID_ARG, "lambda_t must be > 0");
+    if (dev_rgb_prev && !dev_rgb_cur) return fail(ctx, GGT_ERR_INVALID_ARG, "rgb_prev given without rgb_cur");
+    const long long cells = (long long)((width + 3) / 4) * ((height + 3) / 4);
+    if (cells > GGT_REFINE_STATIC_MAX_CELLS)
+        return fail(ctx, GGT_ERR_SHAPE, "ggt_refine_depth_static: %dx%d needs %lld quarter-resolution cells, the fixed scratch holds %d "
+                    "(use ggt_refine_depth)", width, height, cells, GGT_REFINE_STATIC_MAX_CELLS);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!dev_rgb_prev) {                                        // first-frame rule (M = 1): no scratch involved
+        cudaError_t e = ggt_launch_first_frame(width, height, dev_depth_cur, dev_depth_state, dev_mask_out, st);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "ggt_refine_depth_static first-frame launch");
+        ctx->launches += 1;
+        return GGT_OK;
+    }
+    uint16_t* cq = nullptr;
+    cudaError_t e = ggt_refine_static_scratch(&cq);
+    if (e != cudaSuccess || !cq) return cuda_fail(ctx, e, "address of the fixed refine scratch");
+    GgtRefineViews tab;
+    memset(&tab, 0, sizeof tab);
+    tab.n = 1;
+    tab.v[0].rgb_cur = dev_rgb_cur; tab.v[0].rgb_prev = dev_rgb_prev; tab.v[0].depth_cur = dev_depth_cur;
+    tab.v[0].depth_state = dev_depth_state; tab.v[0].mask_out = dev_mask_out; tab.v[0].pooled_out = dev_pooled_out;
+    tab.v[0].cq = cq;
+    int n = 0;
+    e = ggt_launch_refine(width, height, tab, rgb_pixel_stride, params->lambda_t, params->beta, params->theta, st, &n);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "ggt_refine_depth_static launch");
+    ctx->launches += n;
+    return GGT_OK;
+}
+
 // a3: validates the views, sizes the {depth, omega} workspace and launches the weight-map pre-pass for all of them
 // (one launch); map_out[k] is the device address of view k's zero-padded {depth, omega} map.
 static int prepare_maps(ggt_ctx* ctx, int32_t n_views, const ggt_camera* views, const float* const* dev_depths,

@@ -208,6 +208,7 @@ static inline int ggt_group_of(int dtype) { return dtype == GGT_F16 ? 8 : 4; }
 // ---- kernel launchers (each returns cudaError_t of the launch) ----------------------------------------
 cudaError_t ggt_launch_refine(int W, int H, const GgtRefineViews& tab, int stride, float lambda_t, float beta, float theta,
                               cudaStream_t st, int* n_launches);
+cudaError_t ggt_refine_static_scratch(uint16_t** ptr);   // ggt_refine.cu: address of the fixed-size scratch on this device
 cudaError_t ggt_launch_first_frame(int W, int H, const float* depth_cur, float* depth_state, float* mask_out, cudaStream_t st);
 cudaError_t ggt_launch_weight_maps(const GgtWeightParams& p, cudaStream_t st);
 cudaError_t ggt_launch_integrate(const GgtIntegrateParams& p, int dtype, bool fused, int sm_count, cudaStream_t st);

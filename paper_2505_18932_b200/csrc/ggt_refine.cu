@@ -13,6 +13,8 @@
 // HBM traffic per pixel: 6 B colour + 12 B depth (+4 B mask if requested) -> streaming, HBM-bound.
 #include "ggt_internal.h"
 
+#include <mutex>
+
 namespace {
 
 constexpr int S = 4;           // quarter resolution per axis (reading P7)
@@ -189,6 +191,19 @@ k_first_frame(size_t n, const float* __restrict__ depth_cur, float* __restrict__
     if (mask_out) mask_out[i] = 1.0f;
 }
 
+// ---- ggt_refine_depth_static: the block-difference scratch without an allocation -----------------------------------
+// The one piece of scratch memory of the refine step (k_block_diff's quarter-resolution L1 differences, read back by
+// k_mask_blend) as a file-scope device array of a fixed size, for callers that may not allocate (stream capture, serving
+// loops).  512 KB: quarter-resolution cells of one view of up to 2048 x 2048 pixels (1920 x 1080 needs 259 200 B); every
+// GPU that loads the library holds it until the process exits.  All calls share it.
+__device__ __align__(256) uint16_t g_refine_static_cq[GGT_REFINE_STATIC_MAX_CELLS];
+
+// In host code `g_refine_static_cq` is only a handle of the symbol, not a device address: the address is asked for once
+// per device, with that device current, and kept.
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mutex;
+uint16_t* g_static_ptr[kMaxDevices] = {};
+
 }  // namespace
 
 // All views of `tab` have the same size and a previous colour image; one launch of each kernel, blockIdx.z = view.
@@ -218,4 +233,21 @@ cudaError_t ggt_launch_first_frame(int W, int H, const float* depth_cur, float* 
     const size_t n = (size_t)W * H;
     k_first_frame<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, depth_cur, depth_state, mask_out);
     return cudaGetLastError();
+}
+
+// Device address of the static scratch on the CURRENT device (cached per device; no allocation).
+cudaError_t ggt_refine_static_scratch(uint16_t** ptr) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        void* a = nullptr;
+        e = cudaGetSymbolAddress(&a, g_refine_static_cq);
+        if (e != cudaSuccess) return e;
+        g_static_ptr[dev] = static_cast<uint16_t*>(a);
+    }
+    *ptr = g_static_ptr[dev];
+    return cudaSuccess;
 }
