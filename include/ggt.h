@@ -20,6 +20,11 @@
  *     validate host-side arguments synchronously, enqueue kernels on `stream` and return WITHOUT
  *     synchronising.  No exception crosses the ABI.
  *   - there is no CPU fallback: without a CUDA device every compute call returns GGT_ERR_CUDA.
+ *   - stream capture: the compute calls only launch kernels on `stream` (arguments travel as kernel parameters), so a
+ *     frame can be captured into a CUDA graph and replayed, provided nothing has to grow during capture: reserve the
+ *     {depth, omega} workspace first (ggt_set_workspace, or one eager call of the same shape), refine with
+ *     ggt_refine_depth_static (or after one eager ggt_refine_depth* call of the same shape), leave stage profiling off,
+ *     and keep ggt_volume_bind, ggt_splat_reserve and ggt_frame_host (which owns streams and events) outside the capture.
  *   - depth maps hold z-depth in metres (the quantity Eq. 9 compares with z_k); <= 0 means invalid.
  *   - pixel (i, j) has its centre at (i + 0.5, j + 0.5); images are row-major, row 0 on top.
  *   - arithmetic is IEEE fp32 in a fixed operation order (P14), so
