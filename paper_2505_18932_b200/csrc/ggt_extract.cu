@@ -69,6 +69,9 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
     bool found = !live || h_end <= h_first;
     const int g_start = max((int)__reduce_min_sync(0xffffffffu, found ? 0xffffu : (unsigned)h_first) - 1, 0) / UNROLL * UNROLL;
     const int g_end = (int)__reduce_max_sync(0xffffffffu, found ? 0u : (unsigned)h_end);
+    // the far bin of a crossing lies inside this ray's own range: groups past it are loaded only for other rays of the
+    // warp, or not at all (zero words), and must not end a positive run of this ray
+    const int j_lim = min(p.D, h_end * G);
     float pT = 0.0f;
     float out_d = 0.0f, out_c = 0.0f;
     int out_b = -1;
@@ -79,7 +82,7 @@ k_extract(const __grid_constant__ GgtExtractParams p) {
 #pragma unroll
         for (int i = 0; i < G; ++i) {
             const int j = j0 + i;
-            if (!found && pT > 0.0f && !(T[i] > 0.0f) && j < p.D) {
+            if (!found && pT > 0.0f && !(T[i] > 0.0f) && j < j_lim) {
                 const float Wa = weight_at<HALF>(wpl, plane, j - 1), Wb = weight_at<HALF>(wpl, plane, j);
                 if (Wa > 0.0f && Wb > 0.0f) {
                     const float pz = s_z[j - 1], z = s_z[j];

@@ -345,3 +345,125 @@ def test_extract_after_reset_fused_and_large_unsplit_launches():
             assert np.array_equal(d.cpu().numpy().view(np.uint32), ed.view(np.uint32))
             assert np.array_equal(c.cpu().numpy().view(np.uint32), ec.view(np.uint32))
     assert (ob >= 0).mean() > 0.5 and (ob < 0).any()
+
+
+# ---- bins that no view can see: the march hands them to the tail alone (exact skip in k_integrate) ------------------
+def _unseen_fraction(tgt, views, z):
+    """Oracle-side: fraction of (ray, bin) no view sees, and of 32-pixel row segments that are seen only in part."""
+    uc, vc = np.meshgrid(np.arange(tgt.width) + 0.5, np.arange(tgt.height) + 0.5)
+    seen = np.zeros((tgt.height, tgt.width, z.size), bool)
+    for cam in views:
+        Hm, e = oracle.relative(tgt, cam)
+        b = [Hm[r, 0] * uc + Hm[r, 1] * vc + Hm[r, 2] for r in range(3)]
+        x, y, w = [z[None, None, :] * b[r][..., None] + e[r] for r in range(3)]
+        with np.errstate(divide="ignore", invalid="ignore"):
+            seen |= (w > 1e-6) & (x / w >= 0) & (x / w < cam.width) & (y / w >= 0) & (y / w < cam.height)
+    nw = tgt.width // 32
+    seg = seen[:, :nw * 32].reshape(tgt.height, nw, 32, z.size).any(axis=2)           # row segment x bin
+    part = (seg.any(axis=2) & ~seg.all(axis=2)).mean()
+    return 1.0 - seen.mean(), part, (~seg.any(axis=2)).mean()
+
+
+@pytest.mark.parametrize("dtype_name,accumulate,fused", [("f32", False, False), ("f16", False, False), ("f32", True, False),
+                                                          ("f16", True, False), ("f32", False, True), ("f16", True, True)])
+@pytest.mark.parametrize("rig_kind", ["parallel", "rotated", "across"])
+def test_target_looks_past_the_rig(dtype_name, accumulate, fused, rig_kind):
+    """A 110-degree target yawed away from a narrow rig: whole row segments see no view at all, others only over part of
+    their bins (near end, far end, or -- views looking across the frustum -- only a middle stretch).  Frame 0 uses a
+    narrow target that every view covers, so in overwrite mode the unseen bins of the later frames must be cleared over
+    stale data, and in persistent mode they decay."""
+    import torch
+    from paper_2505_18932_b200 import binding
+    wl = synth.workload("C2", scale=0.2)
+    W, H, D = 200, 41, 48 if dtype_name == "f32" else 56
+    rig = synth.grid_rig(W, H)
+    if rig_kind == "parallel":
+        views = [rig[5], rig[6], rig[9], rig[10]]
+    elif rig_kind == "rotated":
+        views = [synth.camera_from_pose(c.centre, synth.rot_yaw_pitch(0.03 * (i - 1), 0.02 * i), c.fx, c.fy, c.cx, c.cy, c.width, c.height)
+                 for i, c in enumerate([rig[5], rig[6], rig[9]])]
+    else:
+        views = [synth.camera_from_pose((-1.2, 0.0, 1.6), synth.rot_yaw_pitch(math.radians(-75.0), 0.0), rig[5].fx, rig[5].fy, rig[5].cx,
+                                        rig[5].cy, W, H),
+                 synth.camera_from_pose((1.1, 0.1, 2.4), synth.rot_yaw_pitch(math.radians(70.0), 0.0), rig[5].fx, rig[5].fy, rig[5].cx,
+                                        rig[5].cy, W, H)]
+    narrow = synth.camera_from_pose((0.02, 0.01, 0.0), np.eye(3), 0.8 * W, 0.8 * W, W / 2, H / 2, W, H)
+    wide = [synth.camera_from_pose((0.02, 0.01, 0.0), synth.rot_yaw_pitch(math.radians(a), math.radians(4.0)), 0.35 * W, 0.35 * W,
+                                   W / 2, H / 2, W, H) for a in (25.0, -32.0)]
+    targets = [narrow, wide[0], wide[1]]
+    z = synth.bins_inverse(0.5, 5, D)
+    tau = oracle.tau_table(z, 2.0)
+    for t in wide:
+        unseen, part, none = _unseen_fraction(t, views, z)
+        assert unseen > 0.3 and part > 0.1, (unseen, part, none)
+        if rig_kind != "across":
+            assert none > 0.1, (unseen, part, none)
+    ctx = binding.Context()
+    vol = ctx.ggt_volume_bind(W, H, z, dtype=binding.GGT_F16 if dtype_name == "f16" else binding.GGT_F32, weight_cap=0.3, decay=0.9)
+    vol.ggt_volume_reset()
+    T = Wt = None
+    n = W * H
+    for f, tgt in enumerate(targets):
+        depths = _scene_depths(views, wl.scene, 77, f)
+        maps = [oracle.weight_map(d) for d in depths]
+        T, Wt = oracle.integrate(tgt, z, tau, views, maps, T=T if accumulate else None, Wt=Wt if accumulate else None,
+                                 accumulate=accumulate, decay=0.9, cap=0.3, half_storage=dtype_name == "f16")
+        od, oc, ob = oracle.extract(z, T, Wt)
+        gd = [torch.from_numpy(np.ascontiguousarray(d)).cuda() for d in depths]
+        depth = torch.empty(n, dtype=torch.float32, device="cuda")
+        conf = torch.empty(n, dtype=torch.float32, device="cuda")
+        bins = torch.empty(n, dtype=torch.int32, device="cuda")
+        flags = binding.GGT_ACCUMULATE if accumulate else binding.GGT_OVERWRITE
+        if fused:
+            ctx.ggt_integrate_extract(vol, tgt, views, gd, flags, depth, conf, bins)
+        else:
+            ctx.ggt_integrate(vol, tgt, views, gd, flags)
+            ctx.ggt_extract_depth(vol, depth, conf, bins)
+        st = helpers.compare_frame(dict(rays=None, T=T, W=Wt, depth=od, conf=oc, bins=ob),
+                                   dict(vol=vol, depth=depth, conf=conf, bins=bins), z, tau, label="frame %d" % f)
+        helpers.assert_parity(st)
+        assert st["T_bitexact"] and st["W_bitexact"] and st["bin_equal"], st
+    assert (Wt > 0).mean() > 0.003 and (accumulate or (Wt == 0).mean() > 0.3)
+
+
+def test_unseen_bins_large_image_all_view_counts():
+    """1080p-wide rows (several CTAs per row, one unsplit launch) with a wide target, V = 1 ... 9, overwrite over a stale
+    volume: sampled rays against the oracle."""
+    import torch
+    from paper_2505_18932_b200 import binding
+    wl = synth.workload("C2", scale=0.5)
+    W, H, D = 960, 270, 64
+    rig = synth.grid_rig(W, H)
+    z = synth.bins_inverse(0.5, 5, D)
+    tau = oracle.tau_table(z, 2.0)
+    narrow = synth.camera_from_pose((0.0, 0.0, 0.0), np.eye(3), 0.8 * W, 0.8 * W, W / 2, H / 2, W, H)
+    wide = synth.camera_from_pose((0.03, 0.0, 0.0), synth.rot_yaw_pitch(math.radians(20.0), 0.0), 0.4 * W, 0.4 * W, W / 2, H / 2, W, H)
+    rays = helpers.sample_rays(W, H, 16, 4321)
+    ctx = binding.Context()
+    vol = ctx.ggt_volume_bind(W, H, z)
+    n = W * H
+    for V in (1, 2, 3, 4, 5, 6, 7, 8, 9):
+        views = [rig[i] for i in synth.nearest_views(narrow, rig, V)]
+        depths = _scene_depths(views, wl.scene, 99, V)
+        gd = [torch.from_numpy(np.ascontiguousarray(d)).cuda() for d in depths]
+        ctx.ggt_integrate(vol, narrow, views, gd, binding.GGT_OVERWRITE)              # stale content everywhere
+        maps = [oracle.weight_map(d) for d in depths]
+        T, Wt = oracle.integrate(wide, z, tau, views, maps, rays=rays)
+        od, oc, ob = oracle.extract(z, T, Wt)
+        depth = torch.empty(n, dtype=torch.float32, device="cuda")
+        conf = torch.empty(n, dtype=torch.float32, device="cuda")
+        bins = torch.empty(n, dtype=torch.int32, device="cuda")
+        ctx.ggt_integrate(vol, wide, views, gd, binding.GGT_OVERWRITE)
+        ctx.ggt_extract_depth(vol, depth, conf, bins)
+        st = helpers.compare_frame(dict(rays=rays, T=T, W=Wt, depth=od, conf=oc, bins=ob),
+                                   dict(vol=vol, depth=depth, conf=conf, bins=bins), z, tau, label="V = %d" % V)
+        helpers.assert_parity(st)
+        assert st["T_bitexact"] and st["W_bitexact"] and st["bin_equal"], st
+        assert (Wt == 0).mean() > 0.2
+        # every ray: ggt_extract_depth against the oracle's search on the exported volume.  (With one view some rays run
+        # - - + + to the end of their search range: the zero words past a ray's range must not end that positive run.)
+        Tg, Wg = vol.ggt_volume_export()
+        od2, oc2, ob2 = oracle.extract(z, Tg.cpu().numpy(), Wg.cpu().numpy())
+        assert np.array_equal(bins.cpu().numpy(), ob2), "V = %d: %d rays" % (V, int((bins.cpu().numpy() != ob2).sum()))
+        assert np.array_equal(depth.cpu().numpy().view(np.uint32), od2.view(np.uint32))
+        assert np.array_equal(conf.cpu().numpy().view(np.uint32), oc2.view(np.uint32))
