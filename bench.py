@@ -337,6 +337,15 @@ def roofline_of(inp, prof, stage_ms, fused, hbm_peak, peak_src, peaks):
             tj = json.load(fh)
         roof["traffic"] = tj.get(wl.name + ("_fused" if fused else ""))
         roof["traffic_source"] = "profiles/traffic_integrate.json (ncu --set full capture of this kernel; not measured in this run)"
+        if roof["traffic"] and integ_ms > 0:
+            # DRAM bytes actually moved over this run's kernel time: k_integrate leaves out what it can prove away (views
+            # that cannot see a stretch of bins; plane words of unseen bins whose bits do not change are not rewritten), so
+            # on wide-angle targets it moves fewer bytes than the algorithmic count and `frac` is an effective rate
+            roof["dram_frac"] = roof["traffic"] / (integ_ms / 1e3) / 1e9 / hbm_peak
+            if roof["traffic"] < 0.9 * integ_bytes:
+                roof["note"] = ("the kernel moves %.2f GB per launch against %.2f GB algorithmic (bins that no view sees and that were "
+                                "never observed are read but not rewritten): frac is an effective rate, dram_frac the real one"
+                                % (roof["traffic"] / 1e9, integ_bytes / 1e9))
         wi = tj.get(wl.name + "_warp_instructions")
         if wi and not fused and integ_ms > 0:
             # the kernel's practical limit: one warp instruction per SM sub-partition per clock; the instruction count is
