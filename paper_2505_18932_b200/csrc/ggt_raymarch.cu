@@ -169,11 +169,8 @@ __device__ __forceinline__ void march_ray(const GgtRaymarchParams& p, int u, int
     if (p.steps) p.steps[o] = n;
 }
 
-#ifndef GGT_RM_CTAS
-#define GGT_RM_CTAS 4
-#endif
 template <int NV>
-__global__ void __launch_bounds__(256, GGT_RM_CTAS)
+__global__ void __launch_bounds__(256, 4)
 k_raymarch(const __grid_constant__ GgtRaymarchParams p) {
     const int u_raw = blockIdx.x * 32 + threadIdx.x;
     const int v = blockIdx.y * 8 + threadIdx.y;
