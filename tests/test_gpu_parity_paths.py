@@ -467,3 +467,39 @@ def test_unseen_bins_large_image_all_view_counts():
         assert np.array_equal(bins.cpu().numpy(), ob2), "V = %d: %d rays" % (V, int((bins.cpu().numpy() != ob2).sum()))
         assert np.array_equal(depth.cpu().numpy().view(np.uint32), od2.view(np.uint32))
         assert np.array_equal(conf.cpu().numpy().view(np.uint32), oc2.view(np.uint32))
+
+
+@pytest.mark.parametrize("seed", list(range(16)))
+def test_random_rigs_and_targets_bit_exact(seed):
+    """Random geometry against the oracle, every voxel: the exact-skip logic of k_integrate (visible_z, the per-view stretches
+    on rigs of identical parallel cameras, the unseen groups) must never drop a sample that the oracle uses.  Even seeds:
+    identical parallel cameras at random coplanar centres (shared H and w) under a randomly rotated, randomly wide target;
+    odd seeds: every view rotated on its own, with its own focal length and (seed % 4 == 3) its own size."""
+    rng = np.random.default_rng(9000 + seed)
+    wl = synth.workload("C2", scale=0.2)
+    W, H = int(rng.integers(70, 140)), int(rng.integers(24, 48))
+    V = int(rng.integers(2, 7))
+    D = int(rng.integers(18, 44))
+    dtype_name = "f16" if seed % 3 == 0 else "f32"
+    accumulate, fused = bool(seed % 5 == 1), bool(seed % 4 == 2)
+    f_t = float(rng.uniform(0.3, 1.1)) * W
+    tgt = synth.camera_from_pose(tuple(rng.uniform(-0.15, 0.15, 3)), synth.rot_yaw_pitch(float(rng.uniform(-0.6, 0.6)), float(rng.uniform(-0.25, 0.25))),
+                                 f_t, f_t, W / 2 + float(rng.uniform(-5, 5)), H / 2 + float(rng.uniform(-3, 3)), W, H)
+    views = []
+    if seed % 2 == 0:
+        R = synth.rot_yaw_pitch(float(rng.uniform(-0.2, 0.2)), float(rng.uniform(-0.1, 0.1)))
+        f_v = float(rng.uniform(0.6, 1.0)) * W
+        for k in range(V):
+            off = R.T @ np.array([rng.uniform(-0.6, 0.6), rng.uniform(-0.3, 0.3), 0.0])      # coplanar, plane normal = the optical axis
+            views.append(synth.camera_from_pose(tuple(off), R, f_v, f_v, W / 2, H / 2, W, H))
+    else:
+        for k in range(V):
+            Wk, Hk = (W + 8 * (k % 3), H + 4 * (k % 2)) if seed % 4 == 3 else (W, H)
+            f_v = float(rng.uniform(0.5, 1.2)) * Wk
+            views.append(synth.camera_from_pose(tuple(rng.uniform(-0.7, 0.7, 3) * np.array([1.0, 0.5, 0.3])),
+                                                synth.rot_yaw_pitch(float(rng.uniform(-0.5, 0.5)), float(rng.uniform(-0.2, 0.2))),
+                                                f_v, f_v, Wk / 2, Hk / 2, Wk, Hk))
+    z = synth.bins_inverse(0.5, 5, D) if seed % 2 else synth.bins_uniform(0.6, 4.5, D)
+    st, T, Wt, ob = run_case(tgt, views, z, lambda f: _scene_depths(views, wl.scene, 500 + seed, f), frames=2 if accumulate else 1,
+                             dtype_name=dtype_name, accumulate=accumulate, fused=fused, weight_cap=0.4, decay=0.85)
+    assert st["T_bitexact"] and st["W_bitexact"] and st["bin_equal"], st
