@@ -4,7 +4,7 @@ nvcc cross-compiles without a GPU.  Flags that matter for correctness: --fmad=fa
 contraction: every fused multiply-add in the kernels is an explicit fmaf, P14), default
 -prec-div / -prec-sqrt / no -ftz (IEEE), -Xcompiler -ffp-contract=off for the host-side camera algebra.
 Each source is compiled to an object file in its own nvcc process (in parallel); ggt_integrate.cu, whose
-kernel instantiations dominate the compile time, four times, once per storage / mode variant.
+kernel instantiations dominate the compile time, eight times, once per storage / mode / fusion variant.
 """
 from __future__ import annotations
 
@@ -20,7 +20,7 @@ LIB = os.path.join(HERE, "libggt.so")
 # (source, extra defines)
 UNITS = [("ggt_api.cu", []), ("ggt_refine.cu", []), ("ggt_weight.cu", []), ("ggt_extract.cu", []),
          ("ggt_raymarch.cu", []), ("ggt_temporal.cu", []), ("ggt_features.cu", []), ("ggt_splat.cu", [])] + \
-        [("ggt_integrate.cu", ["-DGGT_INTEGRATE_VARIANT=%d" % v]) for v in range(4)]
+        [("ggt_integrate.cu", ["-DGGT_INTEGRATE_VARIANT=%d" % v]) for v in range(8)]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--fmad=false", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math"]
 
