@@ -15,6 +15,7 @@ ggt_refine_depth on each of the V views, ggt_integrate (weight maps + fusion), g
 """
 import argparse
 import json
+import math
 import os
 import sys
 import threading
@@ -602,6 +603,22 @@ def main():
         ms_f = timed(torch, None, fused_fn, k, 3) / k
         extra["fused_integrate_extract"] = {"ms_per_call": ms_f, "includes": "weight maps + fused integrate/extract kernel (no volume re-read)",
                                             "gvoxel_view_per_s": inp.vv_per_step / (ms_f / 1e3) / 1e9}
+        # the same inputs seen by cameras that do NOT share H (a real rig: every camera with its own rotation): view i
+        # yawed by 4 (i - 1.5) degrees, every second one pitched by 2 degrees.  The cameras only change the projection the
+        # kernel evaluates (the depth maps stay those of the parallel rig: this leg times the march, it renders nothing)
+        from paper_2505_18932_b200 import synth as _synth
+        turned = [_synth.camera_from_pose(c.centre, _synth.rot_yaw_pitch(math.radians(4.0 * (i - 1.5)), math.radians(2.0 * (i % 2))),
+                                          c.fx, c.fy, c.cx, c.cy, c.width, c.height) for i, c in enumerate(inp.views)]
+        np_fn = lambda: dev.ctx.ggt_integrate(dev.vol, inp.target, turned, depths, dev.flags)
+        for _ in range(3):                                       # the first launch of this kernel loads it
+            np_fn()
+        dev.ctx.ggt_profile_enable(True)
+        timed(torch, None, np_fn, k, 0)
+        prof_n = dev.ctx.ggt_profile_collect()
+        dev.ctx.ggt_profile_enable(False)
+        extra["non_parallel_rig"] = {"call": "ggt_integrate on the step's inputs with every view rotated on its own (no shared H: per-view w and 1/w)",
+                                     "k_integrate_ms_per_launch": prof_n["integrate"][0] / max(prof_n["integrate"][1], 1),
+                                     "parallel_rig_k_integrate_ms_per_launch": integ_ms}
         n_t = t.width * t.height
         steps_out = torch.zeros(n_t, dtype=torch.int32, device="cuda")
         zn, zf = float(wl.z_bins[0]), float(wl.z_bins[-1])
